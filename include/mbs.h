@@ -1,0 +1,163 @@
+/*
+ * mbs.h -- C ABI of the B200-native modified-Born-series (MBS) Helmholtz solver with the
+ * non-overlapping domain decomposition of Mache & Vellekoop, arXiv 2410.02395.
+ *
+ * Citations "P:NN" are line numbers of PAPER.md (the paper text); "R<k>" are the readings of
+ * points the paper leaves open, listed in DESIGN.md section 3.
+ *
+ * The library solves   [nabla^2 + k^2(r)] x(r) = -y(r)            (Eq. (1))
+ * on a regular 1D/2D/3D grid with the preconditioned Richardson iteration
+ *     x <- x - alpha B ( x - (L+I)^-1 [ y_vec + B x ] ),  B = I - V     (Eq. (6))
+ * where L is a per-subdomain FFT convolution (Eq. (8)) and V holds the scattering
+ * potential plus the truncated wrap-around / transfer corrections.
+ *
+ * Conventions
+ *  - All arrays are complex64 (interleaved float re, im), C order, axis 0 slowest, `shape` voxels.
+ *  - "device" pointers are CUDA device pointers, 16-byte aligned; "host" pointers are ordinary
+ *    host memory.  The caller owns every array it passes in; the library owns the context and
+ *    (unless mbs_set_workspace is used) its workspace.
+ *  - Every call returns an int status (MBS_OK = 0).  No exceptions cross the boundary, there is
+ *    no global state, and one context must be used from one thread at a time.
+ *  - All device work is enqueued on the stream given to mbs_create.  mbs_apply_operator and
+ *    mbs_set_potential are asynchronous with respect to the host unless stated; mbs_solve*
+ *    return after the stop decision has been observed.
+ *  - There is no CPU fallback: every step runs in the library's CUDA kernels (sm_100a).
+ */
+#ifndef MBS_B200_H
+#define MBS_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define MBS_API __attribute__((visibility("default")))
+#else
+#define MBS_API
+#endif
+
+typedef struct mbs_ctx mbs_ctx;
+
+enum mbs_status {
+    MBS_OK = 0,
+    MBS_ERR_INVALID_ARG = 1,      /* bad argument; see mbs_last_error                       */
+    MBS_ERR_UNSUPPORTED_SIZE = 2, /* a subdomain length has no FFT plan (see mbs_fft_supported) */
+    MBS_ERR_OOM = 3,              /* device or host allocation failed                        */
+    MBS_ERR_CUDA = 4,             /* CUDA runtime error; text in mbs_last_error              */
+    MBS_ERR_NOT_CONVERGED = 5,    /* max_iter reached; x and the history are still valid     */
+    MBS_ERR_NUMERIC = 6,          /* NaN/Inf in the residual                                 */
+    MBS_ERR_STATE = 7             /* call out of order (e.g. solve before set_potential)     */
+};
+
+/* Operators of mbs_apply_operator.  All are the SCALED operators (they include c). */
+enum mbs_operator {
+    MBS_OP_B = 0,          /* B = I - V: scattering diagonal + edge-slab corrections */
+    MBS_OP_PROPAGATOR = 1, /* (L+I)^-1: per-subdomain FFT, 1/(c(k0^2-|p|^2)+1), inverse FFT */
+    MBS_OP_A = 2,          /* A = (L+I) - B                                            */
+    MBS_OP_PRECOND_A = 3   /* Gamma^-1 A = B - B (L+I)^-1 B                            */
+};
+
+/* Options of mbs_set_option. */
+enum mbs_option {
+    MBS_OPT_FUSED = 0,          /* 1 (default): fused sweeps (prologue in the first FFT sweep, epilogue in the
+                                   last, 112 B/voxel-iteration ledger); 0: one kernel per step of P:122-128     */
+    MBS_OPT_CHECK_INTERVAL = 1, /* iterations enqueued between two host polls of the device stop flag (>= 1)  */
+    MBS_OPT_USE_GRAPH = 2       /* 1: replay each poll interval as a CUDA graph (default 1 for small grids)   */
+};
+
+typedef struct mbs_info {
+    double c_re, c_im;             /* scale factor c of Eq. (9)                              */
+    double k02_re, k02_im;         /* background k0^2 (R2)                                           */
+    double v_max;                  /* ||k^2 - k0^2||_inf                                      */
+    double norm_A12;               /* sigma_max(K_t)/h^2 (R5)                                 */
+    int32_t sum_a;                 /* sum_d a_d of Eq. (9)                                   */
+    int32_t ndim;
+    int64_t voxels;
+    int64_t subdomain_shape[3];    /* M_d                                                            */
+    double alpha;                  /* 0.75                                                    */
+    double norm_rhs;               /* ||Gamma^-1 y_vec|| of the last solve                   */
+    double algorithmic_bytes_per_iteration; /* floor ledger of DESIGN.md section 5 (112 B/voxel in 3D) */
+    uint64_t workspace_bytes;
+    int64_t kernel_launches;       /* kernels launched by this context so far                        */
+    double last_solve_ms;          /* device time of the last mbs_solve* iteration loop (CUDA events) */
+} mbs_info;
+
+/*
+ * Create a solver for one grid (P:37-45 problem statement; P:82 decomposition).
+ *  ndim            1, 2 or 3.
+ *  shape[ndim]     grid size in voxels INCLUDING the absorbing layers, axis 0 slowest.
+ *  pixel_size      grid pitch h (same on every axis), same unit as wavelength.   (lambda/4)
+ *  wavelength      vacuum wavelength lambda; k(r) = 2 pi n(r) / lambda.
+ *  boundary_width[ndim]  W_d: thickness in voxels of the absorbing layer on each side (R3).
+ *  n_subdomains[ndim]    S_d >= 1, shape[d] % S_d == 0; subdomain length M_d = shape[d] / S_d.
+ *  periodic[ndim]  1: axis is periodic (no wrap correction when S_d = 1, wrap-around transfer when
+ *                  S_d >= 2); 0: non-periodic.  May be NULL (= all 0).
+ *  n_correction    t: edge points kept in the truncated corrections (paper default 8).
+ *                  0 is legal only if every axis is periodic with S_d = 1.  Requires 2 t <= M_d.
+ *  cuda_stream     a cudaStream_t (may be NULL for the default stream); all work runs on it.
+ * Errors: MBS_ERR_INVALID_ARG, MBS_ERR_UNSUPPORTED_SIZE, MBS_ERR_OOM, MBS_ERR_CUDA.
+ * On failure *out is NULL; mbs_last_error(NULL) returns the reason of the last failed create
+ * on this thread.
+ */
+MBS_API int mbs_create(mbs_ctx** out, int ndim, const int64_t* shape, double pixel_size, double wavelength,
+               const int32_t* boundary_width, const int32_t* n_subdomains, const uint8_t* periodic,
+               int32_t n_correction, void* cuda_stream);
+
+/* 1 if a subdomain length M has an FFT plan in this build (2^a * 5^b sizes listed in DESIGN.md). */
+MBS_API int mbs_fft_supported(int64_t M);
+
+/* Bytes of device workspace the context needs (B_diag, u, slab buffers, reduction scratch). */
+MBS_API size_t mbs_workspace_bytes(const mbs_ctx* ctx);
+
+/* Hand the context a caller-owned device buffer of at least mbs_workspace_bytes (256-byte aligned)
+ * instead of letting it cudaMalloc its own.  Must precede mbs_set_potential.  The buffer must
+ * outlive the context. */
+MBS_API int mbs_set_workspace(mbs_ctx* ctx, void* device_buffer, size_t bytes);
+
+MBS_API int mbs_set_option(mbs_ctx* ctx, int option, int64_t value);
+
+/*
+ * Setup from the complex refractive index n(r) (device, complex64, `shape`):
+ * k^2 = (2 pi/lambda)^2 n^2, absorbing layer (R3), k0^2 (R2), ||k^2-k0^2||_inf, c by Eq. (9),
+ * B_diag = 1 - c (k^2 - k0^2).  Computed in double on the device, stored as complex64.
+ * Requires Im n >= 0 (P:55 convergence condition) -> MBS_ERR_INVALID_ARG otherwise.
+ * The map is read once and not retained.  Synchronises the stream.
+ */
+MBS_API int mbs_set_potential(mbs_ctx* ctx, const void* n_map_device);
+
+/* out = Op(in) for one of enum mbs_operator; device pointers; in == out allowed. */
+MBS_API int mbs_apply_operator(mbs_ctx* ctx, int which, const void* in_device, void* out_device);
+
+/*
+ * Run the iteration of Eq. (6) until eps < tol or max_iter updates (R7, R8).
+ *  y   device, physical source y(r) of Eq. (1); the library forms y_vec = -c y.
+ *  x   device, in/out: x^(0) on entry (zero it for a cold start; any start converges).
+ *  residual_history  host, capacity max_iter (may be NULL): history[n] = eps_n, the relative
+ *      residual ||Gamma^-1(y - A x^(n))|| / ||Gamma^-1 y|| of the iterate BEFORE update n.
+ *  n_iter  host, out: number of updates applied.
+ * Returns MBS_OK (converged), MBS_ERR_NOT_CONVERGED, MBS_ERR_NUMERIC, or a CUDA/state error.
+ */
+MBS_API int mbs_solve(mbs_ctx* ctx, const void* y_device, void* x_device, double tol, int32_t max_iter,
+              double* residual_history, int32_t* n_iter);
+
+/* Same with HOST arrays y and x (complex64, `shape`): copies y and x^(0) to the device, iterates,
+ * copies x back.  The end-to-end entry point (bench.py "e2e"). */
+MBS_API int mbs_solve_host(mbs_ctx* ctx, const void* y_host, void* x_host, double tol, int32_t max_iter,
+                   double* residual_history, int32_t* n_iter);
+
+MBS_API int mbs_get_info(const mbs_ctx* ctx, mbs_info* out);
+
+/* Frees everything the library allocated.  NULL-safe. */
+MBS_API void mbs_destroy(mbs_ctx* ctx);
+
+/* Library-owned text of the last error on this context (or of the last failed mbs_create when
+ * ctx is NULL); valid until the next call on the context. */
+MBS_API const char* mbs_last_error(const mbs_ctx* ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MBS_B200_H */

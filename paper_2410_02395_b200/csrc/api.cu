@@ -1,0 +1,647 @@
+// api.cu -- the C ABI of include/mbs.h: context, host-side setup (Eq. (9), K_t, tables), operator
+// application and the solve loop with its device-side stop flag.  Every step of the hot path runs
+// in the CUDA kernels of kernels.cu / fft_inst.cu; there is no CPU fallback.
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <complex>
+#include <string>
+#include <vector>
+
+#include "mbs_internal.h"
+
+using namespace mbs;
+
+typedef std::complex<double> cd;
+
+struct mbs_ctx {
+    int ndim = 0;
+    int first = 0;  // first real axis of the internal 3-D description
+    GridDesc g{};
+    int W[3] = {0, 0, 0};
+    double h = 0, wavelength = 0;
+    cudaStream_t stream = nullptr;
+    int num_sms = 148;
+
+    // workspace
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    bool ws_owned = false;
+    cf* bdiag = nullptr;
+    cf* u = nullptr;
+    CorrBufs cx{};  // edge corrections of the current operand
+    CorrBufs ds{};  // fused path: d = x - u' at the slab voxels of the non-contiguous axes
+    double* partials = nullptr;
+
+    // small library-owned device data
+    DevState* state = nullptr;
+    double* hist_dev = nullptr;
+    int hist_cap = 0;
+    float* Kh_dev = nullptr;
+    cf* tw_dev[3] = {nullptr, nullptr, nullptr};
+    float* p2_dev[3] = {nullptr, nullptr, nullptr};
+    const FftEntry* fft[3] = {nullptr, nullptr, nullptr};
+    DevState* state_pinned = nullptr;  // 2 slots for polling
+    cudaEvent_t ev_poll[2] = {nullptr, nullptr};
+    cudaEvent_t ev_t0 = nullptr, ev_t1 = nullptr;
+    cf* host_y = nullptr;  // device staging of mbs_solve_host
+    cf* host_x = nullptr;
+
+    // scalars
+    cd c = 0, k02 = 0;
+    double v_max = 0, norm_A12 = 0, beta = 0.5, alpha = 0.75, norm_rhs = 0, last_solve_ms = 0;
+    int sum_a = 0;
+    bool potential_set = false;
+    std::vector<double> Kh;  // t*t
+
+    // options
+    int fused = 0;
+    int check_interval = 0;  // 0 = automatic
+    int use_graph = -1;      // -1 = automatic
+
+    int64_t launches = 0;
+    std::string err;
+};
+
+static thread_local std::string g_create_error;
+
+static int fail(mbs_ctx* ctx, int code, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (ctx) ctx->err = buf;
+    else g_create_error = buf;
+    return code;
+}
+
+#define MBS_CUDA(ctx, expr)                                                                          \
+    do {                                                                                             \
+        cudaError_t e__ = (expr);                                                                    \
+        if (e__ != cudaSuccess)                                                                      \
+            return fail(ctx, e__ == cudaErrorMemoryAllocation ? MBS_ERR_OOM : MBS_ERR_CUDA, "%s: %s", #expr, \
+                        cudaGetErrorString(e__));                                                    \
+    } while (0)
+
+#define MBS_TRY(expr)                    \
+    do {                                 \
+        int rc__ = (expr);               \
+        if (rc__ != MBS_OK) return rc__; \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// host-side small linear algebra: sigma_max of the t x t matrix K_t, cyclic Jacobi on K^T K
+// ---------------------------------------------------------------------------------------------
+static double second_derivative_kernel(int m) {
+    // band-limited second derivative on the infinite grid, units 1/h^2 (R4)
+    if (m == 0) return -M_PI * M_PI / 3.0;
+    return -2.0 * ((m % 2 == 0) ? 1.0 : -1.0) / ((double)m * (double)m);
+}
+
+static double sigma_max(const std::vector<double>& K, int t) {
+    std::vector<double> A((size_t)t * t, 0.0);  // A = K^T K
+    for (int i = 0; i < t; ++i)
+        for (int j = 0; j < t; ++j) {
+            double s = 0;
+            for (int k = 0; k < t; ++k) s += K[(size_t)k * t + i] * K[(size_t)k * t + j];
+            A[(size_t)i * t + j] = s;
+        }
+    for (int sweep = 0; sweep < 100; ++sweep) {
+        double off = 0;
+        for (int i = 0; i < t; ++i)
+            for (int j = i + 1; j < t; ++j) off += A[(size_t)i * t + j] * A[(size_t)i * t + j];
+        if (off < 1e-30) break;
+        for (int p = 0; p < t; ++p)
+            for (int q = p + 1; q < t; ++q) {
+                const double apq = A[(size_t)p * t + q];
+                if (fabs(apq) < 1e-300) continue;
+                const double app = A[(size_t)p * t + p], aqq = A[(size_t)q * t + q];
+                const double theta = (aqq - app) / (2.0 * apq);
+                const double tt = (theta >= 0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+                const double cs = 1.0 / sqrt(tt * tt + 1.0), sn = tt * cs;
+                for (int k = 0; k < t; ++k) {
+                    const double akp = A[(size_t)k * t + p], akq = A[(size_t)k * t + q];
+                    A[(size_t)k * t + p] = cs * akp - sn * akq;
+                    A[(size_t)k * t + q] = sn * akp + cs * akq;
+                }
+                for (int k = 0; k < t; ++k) {
+                    const double apk = A[(size_t)p * t + k], aqk = A[(size_t)q * t + k];
+                    A[(size_t)p * t + k] = cs * apk - sn * aqk;
+                    A[(size_t)q * t + k] = sn * apk + cs * aqk;
+                }
+            }
+    }
+    double mx = 0;
+    for (int i = 0; i < t; ++i) mx = std::max(mx, A[(size_t)i * t + i]);
+    return sqrt(mx);
+}
+
+// ---------------------------------------------------------------------------------------------
+// workspace layout
+// ---------------------------------------------------------------------------------------------
+static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
+
+static size_t corr_elems(const GridDesc& g, int ax) {
+    if (g.a[ax] == 0 || g.t == 0) return 0;
+    return (size_t)(g.voxels / g.N[ax]) * g.S[ax] * 2 * g.t;
+}
+
+static size_t layout_workspace(mbs_ctx* c, char* base) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) {
+        char* p = base ? base + off : nullptr;
+        off += align_up(bytes);
+        return p;
+    };
+    const GridDesc& g = c->g;
+    c->bdiag = (cf*)take(sizeof(cf) * g.voxels);
+    c->u = (cf*)take(sizeof(cf) * g.voxels);
+    for (int ax = 0; ax < 3; ++ax) {
+        const size_t n = corr_elems(g, ax);
+        c->cx.buf[ax] = n ? (cf*)take(sizeof(cf) * n) : nullptr;
+    }
+    for (int ax = 0; ax < 2; ++ax) {
+        const size_t n = corr_elems(g, ax);
+        c->ds.buf[ax] = n ? (cf*)take(sizeof(cf) * n) : nullptr;
+    }
+    c->ds.buf[2] = nullptr;
+    c->partials = (double*)take(sizeof(double) * MBS_MAX_PARTIALS * 5);
+    return off;
+}
+
+// ---------------------------------------------------------------------------------------------
+// create / destroy
+// ---------------------------------------------------------------------------------------------
+extern "C" int mbs_fft_supported(int64_t M) { return (M > 0 && M < (1 << 30) && fft_lookup((int)M)) ? 1 : 0; }
+
+extern "C" int mbs_create(mbs_ctx** out, int ndim, const int64_t* shape, double pixel_size, double wavelength,
+                          const int32_t* boundary_width, const int32_t* n_subdomains, const uint8_t* periodic,
+                          int32_t n_correction, void* cuda_stream) {
+    if (!out) return fail(nullptr, MBS_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (ndim < 1 || ndim > 3) return fail(nullptr, MBS_ERR_INVALID_ARG, "ndim must be 1, 2 or 3 (got %d)", ndim);
+    if (!shape || !boundary_width || !n_subdomains) return fail(nullptr, MBS_ERR_INVALID_ARG, "NULL array argument");
+    if (!(pixel_size > 0) || !(wavelength > 0))
+        return fail(nullptr, MBS_ERR_INVALID_ARG, "pixel_size and wavelength must be positive");
+    if (n_correction < 0) return fail(nullptr, MBS_ERR_INVALID_ARG, "n_correction must be >= 0");
+
+    mbs_ctx* c = new (std::nothrow) mbs_ctx();
+    if (!c) return fail(nullptr, MBS_ERR_OOM, "host allocation failed");
+    c->ndim = ndim;
+    c->first = 3 - ndim;
+    c->h = pixel_size;
+    c->wavelength = wavelength;
+    c->stream = (cudaStream_t)cuda_stream;
+    GridDesc& g = c->g;
+    g.t = n_correction;
+    g.voxels = 1;
+    for (int d = 0; d < 3; ++d) { g.N[d] = g.M[d] = g.S[d] = 1; g.a[d] = 0; g.per[d] = 1; c->W[d] = 0; }
+    int rc = MBS_OK;
+    for (int d = 0; d < ndim && rc == MBS_OK; ++d) {
+        const int ax = c->first + d;
+        const int64_t N = shape[d];
+        const int S = n_subdomains[d], W = boundary_width[d];
+        const int per = periodic ? (periodic[d] ? 1 : 0) : 0;
+        if (N < 1 || N > (1 << 30)) rc = fail(nullptr, MBS_ERR_INVALID_ARG, "shape[%d] = %lld out of range", d, (long long)N);
+        else if (S < 1 || N % S != 0) rc = fail(nullptr, MBS_ERR_INVALID_ARG, "shape[%d] = %lld is not divisible by n_subdomains = %d", d, (long long)N, S);
+        else if (W < 0 || 2 * (int64_t)W > N) rc = fail(nullptr, MBS_ERR_INVALID_ARG, "boundary_width[%d] = %d does not fit in %lld voxels", d, W, (long long)N);
+        else {
+            const int64_t M = N / S;
+            g.N[ax] = (int)N; g.S[ax] = S; g.M[ax] = (int)M; g.per[ax] = per; c->W[ax] = W;
+            g.a[ax] = (S >= 2) ? 2 : (per ? 0 : 1);
+            g.voxels *= N;
+            if (g.a[ax] > 0 && n_correction == 0)
+                rc = fail(nullptr, MBS_ERR_INVALID_ARG, "n_correction = 0 is legal only when every axis is periodic with one subdomain (axis %d is not)", d);
+            else if (g.a[ax] > 0 && 2 * (int64_t)n_correction > M)
+                rc = fail(nullptr, MBS_ERR_INVALID_ARG, "2*n_correction = %d exceeds the subdomain length %lld of axis %d", 2 * n_correction, (long long)M, d);
+            else if (!fft_lookup((int)M))
+                rc = fail(nullptr, MBS_ERR_UNSUPPORTED_SIZE, "no FFT plan for subdomain length %lld (axis %d); supported: 8..1024 powers of two and 40, 80, 160, 320, 640", (long long)M, d);
+            else c->fft[ax] = fft_lookup((int)M);
+        }
+    }
+    if (rc == MBS_OK && g.voxels >= (1LL << 31)) rc = fail(nullptr, MBS_ERR_INVALID_ARG, "grid has %lld voxels; the limit is 2^31 - 1", g.voxels);
+    if (rc != MBS_OK) { delete c; return rc; }
+    c->sum_a = g.a[0] + g.a[1] + g.a[2];
+
+    // K_t / h^2 and ||A_12|| (R4, R5)
+    const int t = g.t;
+    c->Kh.assign((size_t)t * t, 0.0);
+    std::vector<double> K((size_t)t * t);
+    for (int a = 0; a < t; ++a)
+        for (int b = 0; b < t; ++b) K[(size_t)a * t + b] = second_derivative_kernel(t + b - a);
+    for (size_t i = 0; i < K.size(); ++i) c->Kh[i] = K[i] / (pixel_size * pixel_size);
+    c->norm_A12 = t > 0 ? sigma_max(K, t) / (pixel_size * pixel_size) : 0.0;
+
+    auto cleanup_fail = [&](int code, const char* what, cudaError_t e) {
+        g_create_error = std::string(what) + ": " + cudaGetErrorString(e);
+        mbs_destroy(c);
+        return code;
+    };
+    cudaError_t e;
+    int dev = 0;
+    if ((e = cudaGetDevice(&dev)) != cudaSuccess) return cleanup_fail(MBS_ERR_CUDA, "cudaGetDevice", e);
+    if ((e = cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess)
+        return cleanup_fail(MBS_ERR_CUDA, "cudaDeviceGetAttribute", e);
+    if ((e = cudaMalloc(&c->state, sizeof(DevState))) != cudaSuccess) return cleanup_fail(MBS_ERR_OOM, "cudaMalloc(state)", e);
+    if ((e = cudaMemset(c->state, 0, sizeof(DevState))) != cudaSuccess) return cleanup_fail(MBS_ERR_CUDA, "cudaMemset", e);
+    if ((e = cudaMallocHost(&c->state_pinned, 2 * sizeof(DevState))) != cudaSuccess)
+        return cleanup_fail(MBS_ERR_OOM, "cudaMallocHost", e);
+    for (int i = 0; i < 2; ++i)
+        if ((e = cudaEventCreateWithFlags(&c->ev_poll[i], cudaEventDisableTiming)) != cudaSuccess)
+            return cleanup_fail(MBS_ERR_CUDA, "cudaEventCreate", e);
+    if ((e = cudaEventCreate(&c->ev_t0)) != cudaSuccess || (e = cudaEventCreate(&c->ev_t1)) != cudaSuccess)
+        return cleanup_fail(MBS_ERR_CUDA, "cudaEventCreate", e);
+    if (t > 0) {
+        std::vector<float> Kf(c->Kh.begin(), c->Kh.end());
+        if ((e = cudaMalloc(&c->Kh_dev, sizeof(float) * Kf.size())) != cudaSuccess) return cleanup_fail(MBS_ERR_OOM, "cudaMalloc(Kh)", e);
+        if ((e = cudaMemcpy(c->Kh_dev, Kf.data(), sizeof(float) * Kf.size(), cudaMemcpyHostToDevice)) != cudaSuccess)
+            return cleanup_fail(MBS_ERR_CUDA, "cudaMemcpy(Kh)", e);
+    }
+    // twiddle tables W_M^n (double precision, rounded once) and p_d^2 = (2 pi fftfreq(M, h))^2 (R9)
+    for (int ax = c->first; ax < 3; ++ax) {
+        const int M = g.M[ax];
+        std::vector<cf> tw(M);
+        std::vector<float> p2(M);
+        for (int n = 0; n < M; ++n) {
+            const double ang = 2.0 * M_PI * (double)n / (double)M;
+            tw[n] = make_float2((float)cos(ang), (float)(-sin(ang)));
+            const int f = (n < (M + 1) / 2) ? n : n - M;   // numpy fftfreq ordering (Nyquist negative for even M)
+            const double p = 2.0 * M_PI * (double)f / ((double)M * pixel_size);
+            p2[n] = (float)(p * p);
+        }
+        if ((e = cudaMalloc(&c->tw_dev[ax], sizeof(cf) * M)) != cudaSuccess) return cleanup_fail(MBS_ERR_OOM, "cudaMalloc(tw)", e);
+        if ((e = cudaMalloc(&c->p2_dev[ax], sizeof(float) * M)) != cudaSuccess) return cleanup_fail(MBS_ERR_OOM, "cudaMalloc(p2)", e);
+        if ((e = cudaMemcpy(c->tw_dev[ax], tw.data(), sizeof(cf) * M, cudaMemcpyHostToDevice)) != cudaSuccess ||
+            (e = cudaMemcpy(c->p2_dev[ax], p2.data(), sizeof(float) * M, cudaMemcpyHostToDevice)) != cudaSuccess)
+            return cleanup_fail(MBS_ERR_CUDA, "cudaMemcpy(tables)", e);
+    }
+    c->ws_bytes = layout_workspace(c, nullptr);
+    *out = c;
+    return MBS_OK;
+}
+
+extern "C" void mbs_destroy(mbs_ctx* c) {
+    if (!c) return;
+    if (c->ws_owned && c->ws) cudaFree(c->ws);
+    if (c->state) cudaFree(c->state);
+    if (c->hist_dev) cudaFree(c->hist_dev);
+    if (c->Kh_dev) cudaFree(c->Kh_dev);
+    for (int ax = 0; ax < 3; ++ax) {
+        if (c->tw_dev[ax]) cudaFree(c->tw_dev[ax]);
+        if (c->p2_dev[ax]) cudaFree(c->p2_dev[ax]);
+    }
+    if (c->state_pinned) cudaFreeHost(c->state_pinned);
+    for (int i = 0; i < 2; ++i)
+        if (c->ev_poll[i]) cudaEventDestroy(c->ev_poll[i]);
+    if (c->ev_t0) cudaEventDestroy(c->ev_t0);
+    if (c->ev_t1) cudaEventDestroy(c->ev_t1);
+    if (c->host_y) cudaFree(c->host_y);
+    if (c->host_x) cudaFree(c->host_x);
+    delete c;
+}
+
+extern "C" const char* mbs_last_error(const mbs_ctx* c) { return c ? c->err.c_str() : g_create_error.c_str(); }
+
+extern "C" size_t mbs_workspace_bytes(const mbs_ctx* c) { return c ? c->ws_bytes : 0; }
+
+extern "C" int mbs_set_workspace(mbs_ctx* c, void* device_buffer, size_t bytes) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (!device_buffer || bytes < c->ws_bytes) return fail(c, MBS_ERR_INVALID_ARG, "workspace needs %zu bytes, got %zu", c->ws_bytes, bytes);
+    if (((uintptr_t)device_buffer & 255) != 0) return fail(c, MBS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
+    if (c->ws_owned && c->ws) cudaFree(c->ws);
+    c->ws = device_buffer;
+    c->ws_owned = false;
+    layout_workspace(c, (char*)c->ws);
+    c->potential_set = false;
+    return MBS_OK;
+}
+
+static int ensure_workspace(mbs_ctx* c) {
+    if (c->ws) return MBS_OK;
+    MBS_CUDA(c, cudaMalloc(&c->ws, c->ws_bytes));
+    c->ws_owned = true;
+    layout_workspace(c, (char*)c->ws);
+    return MBS_OK;
+}
+
+extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    switch (option) {
+        case MBS_OPT_FUSED: c->fused = value ? 1 : 0; return MBS_OK;
+        case MBS_OPT_CHECK_INTERVAL:
+            if (value < 0 || value > 4096) return fail(c, MBS_ERR_INVALID_ARG, "check interval must be in [0, 4096]");
+            c->check_interval = (int)value;
+            return MBS_OK;
+        case MBS_OPT_USE_GRAPH: c->use_graph = value ? 1 : 0; return MBS_OK;
+        default: return fail(c, MBS_ERR_INVALID_ARG, "unknown option %d", option);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// set_potential (a0 of the scope table)
+// ---------------------------------------------------------------------------------------------
+extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (!n_map_device) return fail(c, MBS_ERR_INVALID_ARG, "n_map is NULL");
+    MBS_TRY(ensure_workspace(c));
+    const GridDesc& g = c->g;
+    SetupParams sp{};
+    sp.n_map = (const cf*)n_map_device;
+    const double kw = 2.0 * M_PI / c->wavelength;
+    sp.kw2 = kw * kw;
+    sp.beta = c->beta;
+    for (int d = 0; d < 3; ++d) sp.W[d] = c->W[d];
+    int nblocks = (int)std::min<long long>((g.voxels + 255) / 256, (long long)std::min(MBS_MAX_PARTIALS, c->num_sms * 8));
+    std::vector<double> host(5 * (size_t)nblocks);
+    MBS_CUDA(c, launch_setup(g, sp, 0, c->partials, nullptr, nblocks, c->stream));
+    MBS_CUDA(c, cudaMemcpyAsync(host.data(), c->partials, sizeof(double) * 5 * nblocks, cudaMemcpyDeviceToHost, c->stream));
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    double mn_re = INFINITY, mx_re = -INFINITY, mn_im = INFINITY, mx_im = -INFINITY, mn_n = INFINITY;
+    for (int b = 0; b < nblocks; ++b) {
+        mn_re = std::min(mn_re, host[5 * b + 0]); mx_re = std::max(mx_re, host[5 * b + 1]);
+        mn_im = std::min(mn_im, host[5 * b + 2]); mx_im = std::max(mx_im, host[5 * b + 3]);
+        mn_n = std::min(mn_n, host[5 * b + 4]);
+    }
+    if (!(mn_re == mn_re) || !std::isfinite(mn_re) || !std::isfinite(mx_re) || !std::isfinite(mx_im))
+        return fail(c, MBS_ERR_NUMERIC, "refractive-index map contains NaN or Inf");
+    if (mn_n < 0.0) return fail(c, MBS_ERR_INVALID_ARG, "Im n < 0 (gain) violates the convergence condition (min Im n = %g)", mn_n);
+    // R2: k0^2 = centre of the bounding box of k^2
+    c->k02 = cd(0.5 * (mn_re + mx_re), 0.5 * (mn_im + mx_im));
+    sp.k02_re = c->k02.real();
+    sp.k02_im = c->k02.imag();
+    MBS_CUDA(c, launch_setup(g, sp, 1, c->partials, nullptr, nblocks, c->stream));
+    MBS_CUDA(c, cudaMemcpyAsync(host.data(), c->partials, sizeof(double) * nblocks, cudaMemcpyDeviceToHost, c->stream));
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    double v2 = 0;
+    for (int b = 0; b < nblocks; ++b) v2 = std::max(v2, host[b]);
+    c->v_max = sqrt(v2);
+    const double denom = c->v_max + (double)c->sum_a * c->norm_A12;   // Eq. (9)
+    if (!(denom > 0)) return fail(c, MBS_ERR_INVALID_ARG, "homogeneous medium without corrections: ||V|| = 0, nothing to scale");
+    c->c = cd(0.0, -0.95 / denom);
+    sp.c_re = c->c.real();
+    sp.c_im = c->c.imag();
+    MBS_CUDA(c, launch_setup(g, sp, 2, nullptr, c->bdiag, nblocks, c->stream));
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->launches += 3;
+    c->potential_set = true;
+    return MBS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// building blocks
+// ---------------------------------------------------------------------------------------------
+static cf to_cf(cd z) { return make_float2((float)z.real(), (float)z.imag()); }
+
+// edge corrections of (in - in2) into c->cx  (a2 / a7 of the scope table)
+static int run_slabs(mbs_ctx* c, const cf* in, const cf* in2, bool in_loop) {
+    for (int ax = 0; ax < 3; ++ax) {
+        if (!c->cx.buf[ax]) continue;
+        SlabParams sp{};
+        sp.in = in; sp.in2 = in2; sp.out = c->cx.buf[ax]; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
+        sp.state = c->state; sp.check_done = in_loop ? 1 : 0;
+        MBS_CUDA(c, launch_slab(c->g, sp, c->stream));
+        c->launches++;
+    }
+    return MBS_OK;
+}
+
+static PointwiseParams pw_defaults(mbs_ctx* c, bool in_loop) {
+    PointwiseParams p{};
+    p.s1 = 1.f; p.s2 = 0.f; p.alpha = (float)c->alpha;
+    p.ysc = make_float2(0.f, 0.f);
+    p.partials = c->partials; p.hist = c->hist_dev; p.state = c->state;
+    p.check_done = in_loop ? 1 : 0;
+    return p;
+}
+
+// (L+I)^-1 (inverse = 1) or (L+I) (inverse = 0) in place on buf  (a3-a5 of the scope table)
+static int run_propagator(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
+    const GridDesc& g = c->g;
+    SymbolParams sp{};
+    const cd ck = c->c * c->k02;
+    sp.A0 = (float)(ck.real() + 1.0);
+    sp.B0 = (float)ck.imag();
+    sp.cr = (float)c->c.real();
+    sp.ci = (float)c->c.imag();
+    sp.scale = (float)(1.0 / ((double)g.M[0] * g.M[1] * g.M[2]));
+    sp.inverse = inverse;
+    const int* done = in_loop ? &c->state->done : nullptr;
+    auto contig = [&](int mode) -> int {
+        ContigGeom cg{};
+        const FftEntry* e = c->fft[2];
+        cg.n_lines = g.voxels / g.M[2];
+        cg.n_tiles = (cg.n_lines + e->C - 1) / e->C;
+        SymbolParams s2 = sp;
+        s2.tab_axis = c->p2_dev[2];
+        MBS_CUDA(c, e->contig(buf, buf, cg, s2, c->tw_dev[2], mode, done, c->num_sms, c->stream));
+        c->launches++;
+        return MBS_OK;
+    };
+    auto strided = [&](int ax, int mode) -> int {
+        const FftEntry* e = c->fft[ax];
+        StridedGeom sg{};
+        long long inner = 1, outer = 1;
+        for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
+        for (int d = 0; d < ax; ++d) outer *= g.N[d];
+        sg.stride = inner; sg.outer_stride = (long long)g.N[ax] * inner; sg.n_outer = (int)outer; sg.n_seg = g.S[ax];
+        sg.inner = (int)inner; sg.tiles_inner = (int)((inner + e->C - 1) / e->C);
+        sg.n_tiles = outer * g.S[ax] * sg.tiles_inner;
+        SymbolParams s2 = sp;
+        s2.tab_axis = c->p2_dev[ax];
+        if (mode == FFT_MID) {
+            // line-invariant part of |p|^2 from the axes after `ax`
+            if (ax == 0) { s2.tabA = c->p2_dev[1]; s2.Ma = g.M[1]; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
+            else { s2.tabA = nullptr; s2.Ma = 1; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
+        }
+        MBS_CUDA(c, e->strided(buf, sg, s2, c->tw_dev[ax], mode, done, c->num_sms, c->stream));
+        c->launches++;
+        return MBS_OK;
+    };
+    if (c->ndim == 1) return contig(FFT_MID);
+    MBS_TRY(contig(FFT_FWD));
+    if (c->ndim == 3) MBS_TRY(strided(1, FFT_FWD));
+    MBS_TRY(strided(c->first, FFT_MID));
+    if (c->ndim == 3) MBS_TRY(strided(1, FFT_INV));
+    return contig(FFT_INV);
+}
+
+// out = s1 * [B_diag (in - in2) + ysc*y - corr(in - in2)] + s2*w
+static int run_B(mbs_ctx* c, const cf* in, const cf* in2, const cf* y, cf ysc, cf* out, float s1, const cf* w, float s2,
+                 int reduce, bool in_loop) {
+    MBS_TRY(run_slabs(c, in, in2, in_loop));
+    PointwiseParams p = pw_defaults(c, in_loop);
+    p.in = in; p.in2 = in2; p.bdiag = c->bdiag; p.y = y; p.ysc = ysc; p.out = out; p.s1 = s1; p.w = w; p.s2 = s2;
+    p.corr = c->cx; p.reduce = reduce;
+    MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
+    c->launches++;
+    return MBS_OK;
+}
+
+// one iteration of Eq. (6), unfused: one kernel per step of P:122-128
+static int run_iteration_unfused(mbs_ctx* c, const cf* y, cf* x) {
+    const cf ysc = to_cf(-c->c);                                                   // y_vec = -c y
+    MBS_TRY(run_B(c, x, nullptr, y, ysc, c->u, 1.f, nullptr, 0.f, RED_NONE, true));  // u = B x + y_vec
+    MBS_TRY(run_propagator(c, c->u, 1, true));                                     // u' = (L+I)^-1 u
+    MBS_TRY(run_slabs(c, x, c->u, true));                                          // corr(x - u')
+    PointwiseParams p = pw_defaults(c, true);                                      // r = B (x - u'); x -= alpha r
+    p.in = x; p.in2 = c->u; p.bdiag = c->bdiag; p.out = x; p.corr = c->cx; p.update = 1; p.reduce = RED_RESIDUAL;
+    MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
+    c->launches++;
+    return MBS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// apply_operator
+// ---------------------------------------------------------------------------------------------
+extern "C" int mbs_apply_operator(mbs_ctx* c, int which, const void* in_device, void* out_device) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
+    if (!in_device || !out_device) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
+    const cf* in = (const cf*)in_device;
+    cf* out = (cf*)out_device;
+    const cf zero = make_float2(0.f, 0.f);
+    switch (which) {
+        case MBS_OP_B:
+            return run_B(c, in, nullptr, nullptr, zero, out, 1.f, nullptr, 0.f, RED_NONE, false);
+        case MBS_OP_PROPAGATOR:
+            if (in != out) MBS_CUDA(c, cudaMemcpyAsync(out, in, sizeof(cf) * c->g.voxels, cudaMemcpyDeviceToDevice, c->stream));
+            return run_propagator(c, out, 1, false);
+        case MBS_OP_A:
+            // A in = (L+I) in - B in
+            MBS_CUDA(c, cudaMemcpyAsync(c->u, in, sizeof(cf) * c->g.voxels, cudaMemcpyDeviceToDevice, c->stream));
+            MBS_TRY(run_propagator(c, c->u, 0, false));
+            return run_B(c, in, nullptr, nullptr, zero, out, -1.f, c->u, 1.f, RED_NONE, false);
+        case MBS_OP_PRECOND_A:
+            // Gamma^-1 A in = B (in - (L+I)^-1 B in)
+            MBS_TRY(run_B(c, in, nullptr, nullptr, zero, c->u, 1.f, nullptr, 0.f, RED_NONE, false));
+            MBS_TRY(run_propagator(c, c->u, 1, false));
+            return run_B(c, in, c->u, nullptr, zero, out, 1.f, nullptr, 0.f, RED_NONE, false);
+        default:
+            return fail(c, MBS_ERR_INVALID_ARG, "unknown operator %d", which);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// solve
+// ---------------------------------------------------------------------------------------------
+static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_iter, double* residual_history,
+                        int32_t* n_iter) {
+    if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
+    if (!y || !x) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
+    if (max_iter < 1) return fail(c, MBS_ERR_INVALID_ARG, "max_iter must be >= 1");
+    if (!(tol >= 0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0");
+    if (n_iter) *n_iter = 0;
+    if (c->hist_cap < max_iter) {
+        if (c->hist_dev) cudaFree(c->hist_dev);
+        c->hist_dev = nullptr;
+        c->hist_cap = 0;
+        MBS_CUDA(c, cudaMalloc(&c->hist_dev, sizeof(double) * (size_t)max_iter));
+        c->hist_cap = max_iter;
+    }
+    DevState init{};
+    init.iter = 0; init.done = 0; init.max_iter = max_iter; init.ticket = 0; init.tol = tol; init.nu2 = 0; init.last_sum = 0;
+    c->state_pinned[0] = init;
+    MBS_CUDA(c, cudaMemcpyAsync(c->state, &c->state_pinned[0], sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
+    // nu = || B (L+I)^-1 y_vec ||
+    MBS_CUDA(c, launch_scale_copy(y, c->u, to_cf(-c->c), c->g.voxels, c->stream));
+    c->launches++;
+    MBS_TRY(run_propagator(c, c->u, 1, false));
+    MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));   // state_pinned[0] is reused below
+
+    int interval = c->check_interval;
+    if (interval <= 0) {
+        interval = (int)std::max<long long>(1, std::min<long long>(64, (4LL << 20) / std::max<long long>(1, c->g.voxels)));
+    }
+    MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
+    int enqueued = 0;
+    int slot = 0;
+    bool pending[2] = {false, false};
+    int final_done = 0;
+    while (true) {
+        // enqueue one batch, then look at the poll of the PREVIOUS batch (one batch of lookahead keeps the GPU busy)
+        const int batch = std::min(interval, max_iter - enqueued);
+        if (batch > 0 && !final_done) {
+            for (int i = 0; i < batch; ++i) MBS_TRY(run_iteration_unfused(c, y, x));
+            enqueued += batch;
+            MBS_CUDA(c, cudaMemcpyAsync(&c->state_pinned[slot], c->state, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
+            MBS_CUDA(c, cudaEventRecord(c->ev_poll[slot], c->stream));
+            pending[slot] = true;
+        }
+        const int prev = slot ^ 1;
+        if (pending[prev]) {
+            MBS_CUDA(c, cudaEventSynchronize(c->ev_poll[prev]));
+            pending[prev] = false;
+            if (c->state_pinned[prev].done) { final_done = c->state_pinned[prev].done; break; }
+        }
+        if (batch <= 0 || enqueued >= max_iter) {
+            // nothing more to enqueue: drain the last poll
+            if (pending[slot]) {
+                MBS_CUDA(c, cudaEventSynchronize(c->ev_poll[slot]));
+                pending[slot] = false;
+                final_done = c->state_pinned[slot].done;
+            }
+            break;
+        }
+        slot ^= 1;
+    }
+    MBS_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    DevState fin{};
+    MBS_CUDA(c, cudaMemcpy(&fin, c->state, sizeof(DevState), cudaMemcpyDeviceToHost));
+    float ms = 0.f;
+    MBS_CUDA(c, cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1));
+    c->last_solve_ms = ms;
+    c->norm_rhs = sqrt(fin.nu2);
+    if (n_iter) *n_iter = fin.iter;
+    if (residual_history && fin.iter > 0)
+        MBS_CUDA(c, cudaMemcpy(residual_history, c->hist_dev, sizeof(double) * (size_t)fin.iter, cudaMemcpyDeviceToHost));
+    if (fin.done == 1) return MBS_OK;
+    if (fin.done == 3) return fail(c, MBS_ERR_NUMERIC, "non-finite residual at iteration %d", fin.iter - 1);
+    return fail(c, MBS_ERR_NOT_CONVERGED, "residual did not reach tol = %g within %d iterations", tol, max_iter);
+}
+
+extern "C" int mbs_solve(mbs_ctx* c, const void* y_device, void* x_device, double tol, int32_t max_iter,
+                         double* residual_history, int32_t* n_iter) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    return solve_device(c, (const cf*)y_device, (cf*)x_device, tol, max_iter, residual_history, n_iter);
+}
+
+extern "C" int mbs_solve_host(mbs_ctx* c, const void* y_host, void* x_host, double tol, int32_t max_iter,
+                              double* residual_history, int32_t* n_iter) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (!y_host || !x_host) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
+    const size_t bytes = sizeof(cf) * (size_t)c->g.voxels;
+    if (!c->host_y) MBS_CUDA(c, cudaMalloc(&c->host_y, bytes));
+    if (!c->host_x) MBS_CUDA(c, cudaMalloc(&c->host_x, bytes));
+    MBS_CUDA(c, cudaMemcpyAsync(c->host_y, y_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    MBS_CUDA(c, cudaMemcpyAsync(c->host_x, x_host, bytes, cudaMemcpyHostToDevice, c->stream));
+    const int rc = solve_device(c, c->host_y, c->host_x, tol, max_iter, residual_history, n_iter);
+    if (rc != MBS_OK && rc != MBS_ERR_NOT_CONVERGED) return rc;
+    const std::string keep = c->err;
+    MBS_CUDA(c, cudaMemcpyAsync(x_host, c->host_x, bytes, cudaMemcpyDeviceToHost, c->stream));
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->err = keep;
+    return rc;
+}
+
+extern "C" int mbs_get_info(const mbs_ctx* c, mbs_info* out) {
+    if (!c || !out) return MBS_ERR_INVALID_ARG;
+    memset(out, 0, sizeof *out);
+    out->c_re = c->c.real(); out->c_im = c->c.imag();
+    out->k02_re = c->k02.real(); out->k02_im = c->k02.imag();
+    out->v_max = c->v_max; out->norm_A12 = c->norm_A12; out->sum_a = c->sum_a; out->ndim = c->ndim;
+    out->voxels = c->g.voxels;
+    for (int d = 0; d < c->ndim; ++d) out->subdomain_shape[d] = c->g.M[c->first + d];
+    out->alpha = c->alpha; out->norm_rhs = c->norm_rhs;
+    const double per_voxel = c->ndim == 3 ? 112.0 : (c->ndim == 2 ? 80.0 : 32.0);
+    out->algorithmic_bytes_per_iteration = per_voxel * (double)c->g.voxels;
+    out->workspace_bytes = c->ws_bytes;
+    out->kernel_launches = c->launches;
+    out->last_solve_ms = c->last_solve_ms;
+    return MBS_OK;
+}

@@ -1,0 +1,28 @@
+// fft_plans.h -- the subdomain lengths M this build has FFT plans for (2^a and 5*2^a), with the
+// points per thread P, the pass radices and the lines per tile C of each.
+// BASELINE.json configs need 128 (cfg 1, 3), 256 (cfg 3, 5), 320 (cfg 4) and 512 (cfg 2, 5).
+#pragma once
+#include "fft_core.cuh"
+
+namespace mbs {
+
+template <int M> struct FftPlan;
+//                                          M     P   radices...
+template <> struct FftPlan<8>    { using type = Plan<8,    8,  8>;            static constexpr int C = 64; };
+template <> struct FftPlan<16>   { using type = Plan<16,   8,  8, 2>;         static constexpr int C = 64; };
+template <> struct FftPlan<32>   { using type = Plan<32,   8,  8, 4>;         static constexpr int C = 32; };
+template <> struct FftPlan<64>   { using type = Plan<64,   8,  8, 8>;         static constexpr int C = 16; };
+template <> struct FftPlan<128>  { using type = Plan<128,  16, 16, 8>;        static constexpr int C = 16; };
+template <> struct FftPlan<256>  { using type = Plan<256,  16, 16, 16>;       static constexpr int C = 16; };
+template <> struct FftPlan<512>  { using type = Plan<512,  16, 16, 16, 2>;    static constexpr int C = 16; };
+template <> struct FftPlan<1024> { using type = Plan<1024, 16, 16, 16, 4>;    static constexpr int C = 8;  };
+template <> struct FftPlan<40>   { using type = Plan<40,   20, 20, 2>;        static constexpr int C = 64; };
+template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        static constexpr int C = 32; };
+template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int C = 16; };
+template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int C = 16; };
+template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int C = 16; };
+
+}  // namespace mbs
+
+#define MBS_FOR_EACH_FFT_SIZE(X) \
+    X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(40) X(80) X(160) X(320) X(640)

@@ -1,0 +1,221 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  Bars (BASELINE.json north_star): relative L2
+<= 1e-5 per operator application; <= 1e-4 on the converged field at the same stopping threshold;
+iteration counts +-1.
+"""
+import numpy as np
+import pytest
+
+from paper_2410_02395_b200 import workloads
+
+pytestmark = pytest.mark.gpu
+
+OP_TOL = 1e-5
+FIELD_TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2410_02395_b200 import binding
+    return binding
+
+
+@pytest.fixture(scope="module")
+def orc():
+    from oracle import mbs_oracle
+    return mbs_oracle
+
+
+def rel(a, b):
+    a = np.asarray(a).astype(np.complex128).ravel()
+    b = np.asarray(b).astype(np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+def make_pair(B, orc, shape, S, W, t, periodic=None, seed=0, medium=None):
+    n = medium if medium is not None else workloads.random_medium(shape, 100 + seed, 1.0, 1.5, 0.02)
+    o = orc.MBSOracle(n, 0.25, 1.0, W, S, periodic=periodic, n_correction=t)
+    s = B.Solver(shape, 0.25, 1.0, W, S, periodic=periodic, n_correction=t)
+    s.set_potential(n)
+    return s, o, n
+
+
+# sizes span several tiles and a ragged tail (transverse extents that are not multiples of the 16-wide tiles)
+OPERATOR_CASES = [
+    # shape, S, W, t, periodic
+    ((256,), (2,), (8,), 8, None),
+    ((640,), (1,), (16,), 8, None),
+    ((128,), (4,), (4,), 8, (1,)),
+    ((128, 80), (2, 1), (8, 8), 8, None),
+    ((64, 96), (1, 3), (4, 4), 4, None),
+    ((80, 128), (2, 2), (4, 0), 8, (0, 1)),
+    ((64, 40, 48), (2, 1, 3), (4, 4, 4), 8, None),
+    ((32, 64, 40), (1, 2, 1), (2, 2, 2), 3, None),     # t = 3 -> generic slab kernel
+    ((16, 32, 128), (2, 2, 2), (2, 2, 2), 4, (1, 0, 0)),
+]
+
+
+@pytest.mark.parametrize("shape,S,W,t,periodic", OPERATOR_CASES)
+def test_operator_parity(B, orc, shape, S, W, t, periodic):
+    s, o, n = make_pair(B, orc, shape, S, W, t, periodic, seed=len(shape))
+    info = s.info()
+    # setup scalars (double on both sides)
+    assert info["c"] == pytest.approx(o.c, rel=1e-12)
+    assert info["k02"] == pytest.approx(o.k02, rel=1e-12)
+    assert info["v_max"] == pytest.approx(o.v_max, rel=1e-12)
+    assert info["norm_A12"] == pytest.approx(o.norm_A12, rel=1e-12)
+    assert info["sum_a"] == sum(o.a)
+    u = workloads.random_field(shape, 7)
+    u128 = u.astype(np.complex128)
+    refs = {
+        B.MBS_OP_B: o.apply_B(u128),
+        B.MBS_OP_PROPAGATOR: o.propagate(u128),
+        B.MBS_OP_A: o.apply_A(u128),
+        B.MBS_OP_PRECOND_A: o.apply_precond_A(u128),
+    }
+    for which, ref in refs.items():
+        got = s.apply_operator(which, u).cpu().numpy()
+        assert rel(got, ref) <= OP_TOL, (which, rel(got, ref))
+    # in == out is allowed
+    import torch
+    ud = torch.from_numpy(u).cuda()
+    s.apply_operator(B.MBS_OP_PRECOND_A, ud, out=ud)
+    assert rel(ud.cpu().numpy(), refs[B.MBS_OP_PRECOND_A]) <= OP_TOL
+    s.close()
+
+
+def test_B_is_diagonal_plus_slabs_only(B, orc):
+    """V touches only the diagonal and the 2t edge points of each subdomain: away from the
+    edges B u = B_diag u exactly as the oracle computes it; at the edges the slab terms are non-zero."""
+    shape, S, W, t = (64, 64, 64), (2, 1, 1), (4, 4, 4), 8
+    s, o, n = make_pair(B, orc, shape, S, W, t, seed=3)
+    u = workloads.random_field(shape, 9)
+    got = s.apply_operator(B.MBS_OP_B, u).cpu().numpy()
+    interior = np.zeros(shape, dtype=bool)
+    interior[8:24, 8:56, 8:56] = True
+    diag_only = (o.B_diag * u.astype(np.complex128))
+    assert rel(got[interior], diag_only[interior]) < 1e-6
+    edge = got[24:32, 8:56, 8:56] - diag_only[24:32, 8:56, 8:56]
+    assert np.abs(edge).max() > 1e-3
+    s.close()
+
+
+SOLVE_CASES = [
+    # name, workload, tol
+    ("cfg1_1d", lambda: workloads.config(1, tol=1e-5), 1),
+    ("cfg2_small", lambda: workloads.config(2, shape=(256, 256), boundary_width=(16, 16), tol=1e-4), 1),
+    ("cfg3_small", lambda: workloads.config(3, shape=(64, 64, 64), boundary_width=(8, 8, 8), tol=1e-3), 1),
+    ("cfg4_small", lambda: workloads.config(4, shape=(80, 80, 80), boundary_width=(8, 8, 8), tol=1e-3), 1),
+    ("cfg5_small", lambda: workloads.config(5, shape=(128, 64, 64), boundary_width=(8, 8, 8), tol=1e-3), 1),
+]
+
+
+@pytest.mark.parametrize("name,make,slack", SOLVE_CASES)
+def test_solve_parity(B, orc, name, make, slack):
+    w = make()
+    n, y = w.make_medium(), w.make_source()
+    o = orc.from_workload(w, n)
+    x_ref, h_ref = o.solve(y, tol=w.tol, max_iter=w.max_iter)
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    x, hist, rc = s.solve(y, tol=w.tol, max_iter=w.max_iter)
+    assert rc == B.MBS_OK
+    assert abs(len(hist) - len(h_ref)) <= slack, (len(hist), len(h_ref))
+    assert hist[0] == pytest.approx(1.0, abs=1e-5)                     # eps_0 = 1 (R8)
+    m = min(len(hist), len(h_ref))
+    # residual history tracks the oracle's while it is well above the complex64 floor
+    k = min(m, 10)
+    assert np.allclose(hist[:k], h_ref[:k], rtol=1e-4)
+    assert rel(x.cpu().numpy(), x_ref) <= FIELD_TOL, rel(x.cpu().numpy(), x_ref)
+    # monotone up to the complex64 rounding floor (relative slack 1e-3)
+    assert np.all(np.diff(hist) <= 1e-3 * hist[:-1])
+    s.close()
+
+
+def test_not_converged_and_warm_start(B, orc):
+    w = workloads.config(1, tol=1e-5)
+    n, y = w.make_medium(), w.make_source()
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    x, hist, rc = s.solve(y, tol=1e-5, max_iter=100)
+    assert rc == B.MBS_ERR_NOT_CONVERGED and len(hist) == 100
+    o = orc.from_workload(w, n)
+    x_ref, h_ref = o.solve(y, tol=0.0, max_iter=100)
+    assert rel(x.cpu().numpy(), x_ref) <= 1e-5
+    assert np.allclose(hist, h_ref, rtol=1e-4)
+    # warm start from the 100-iteration iterate continues the same trajectory
+    x2, hist2, rc2 = s.solve(y, x0=x, tol=1e-5, max_iter=20000)
+    assert rc2 == B.MBS_OK
+    x_full, h_full = o.solve(y, tol=1e-5, max_iter=20000)
+    assert abs((100 + len(hist2)) - len(h_full)) <= 1
+    assert rel(x2.cpu().numpy(), x_full) <= FIELD_TOL
+    s.close()
+
+
+def test_solve_host_matches_device(B):
+    import torch
+    w = workloads.config(2, shape=(128, 128), boundary_width=(8, 8), tol=1e-3)
+    n, y = w.make_medium(), w.make_source()
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    x, hist, rc = s.solve(y, tol=w.tol, max_iter=w.max_iter)
+    yh = torch.from_numpy(y).pin_memory()
+    xh = torch.zeros(w.shape, dtype=torch.complex64).pin_memory()
+    hist2, rc2 = s.solve_host(yh, xh, w.tol, w.max_iter)
+    assert rc2 == rc == B.MBS_OK and len(hist2) == len(hist)
+    assert np.array_equal(xh.numpy(), x.cpu().numpy())          # deterministic reduction, same kernels
+    assert np.array_equal(hist2, hist)
+    s.close()
+
+
+def test_argument_errors(B):
+    with pytest.raises(B.MBSError) as e:
+        B.mbs_create((100,), 0.25, 1.0, (4,), (3,), None, 8)
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
+    with pytest.raises(B.MBSError) as e:
+        B.mbs_create((2 * 88,), 0.25, 1.0, (4,), (2,), None, 8)       # M = 88 has no plan
+    assert e.value.status == B.MBS_ERR_UNSUPPORTED_SIZE
+    with pytest.raises(B.MBSError) as e:
+        B.mbs_create((64,), 0.25, 1.0, (4,), (4,), None, 16)          # 2t > M
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
+    with pytest.raises(B.MBSError) as e:
+        B.mbs_create((64,), 0.25, 1.0, (4,), (1,), None, 0)           # t = 0 on a non-periodic axis
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
+    with pytest.raises(B.MBSError) as e:
+        B.mbs_create((64, 64, 64, 64), 0.25, 1.0, (4,) * 4, (1,) * 4, None, 8)
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
+    # gain medium is rejected
+    s = B.Solver((64,), 0.25, 1.0, (4,), (2,), n_correction=8)
+    n = np.ones(64, dtype=np.complex64)
+    n[10] = 1.2 - 0.1j
+    with pytest.raises(B.MBSError) as e:
+        s.set_potential(n)
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
+    # operator before set_potential
+    s2 = B.Solver((64,), 0.25, 1.0, (4,), (2,), n_correction=8)
+    with pytest.raises(B.MBSError) as e:
+        s2.apply_operator(B.MBS_OP_B, np.zeros(64, dtype=np.complex64))
+    assert e.value.status == B.MBS_ERR_STATE
+    s.close()
+    s2.close()
+
+
+def test_periodic_undecomposed_matches_eq4(B, orc):
+    """t = 0, periodic, one domain: the original MBS of section 2, c from Eq. (4)."""
+    shape = (64, 128)
+    n = workloads.random_medium(shape, 5, 1.0, 1.3, 0.05)
+    o = orc.MBSOracle(n, 0.25, 1.0, (0, 0), (1, 1), periodic=(1, 1), n_correction=0)
+    s = B.Solver(shape, 0.25, 1.0, (0, 0), (1, 1), periodic=(1, 1), n_correction=0)
+    s.set_potential(n)
+    info = s.info()
+    assert info["c"] == pytest.approx(-0.95j / info["v_max"], rel=1e-12)
+    y = np.zeros(shape, dtype=np.complex64)
+    y[10, 20] = 1.0
+    x_ref, h_ref = o.solve(y, tol=1e-4, max_iter=5000)
+    x, hist, rc = s.solve(y, tol=1e-4, max_iter=5000)
+    assert rc == B.MBS_OK and abs(len(hist) - len(h_ref)) <= 1
+    assert rel(x.cpu().numpy(), x_ref) <= FIELD_TOL
+    s.close()
