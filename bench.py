@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the fused MBS iteration (BASELINE.json metric) on N B200s of one node.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3|4|5] [--impl b200|reference]
+
+A "step" is one iteration of Eq. (6) of the paper over the whole grid: every row of
+SURVEY.md 8(a) (scattering operator with edge-slab corrections, per-subdomain FFT propagator, difference,
+second scattering operator, residual norm, alpha-update, stop flag).  The workload is one of the seeded
+synthetic media of BASELINE.json (default: config 5, 1024^3, 4x2x2 subdomains).
+
+Output: ONE JSON line (rank 0).  `value` = voxel-iterations/s with every input resident in HBM, timed with CUDA
+events on the solver's stream, max over ranks; `e2e` = the same metric through the host-buffer entry point
+mbs_solve_host (H2D of y and x0 and D2H of x inside the timed region); `roofline` = the dominant kernel's
+algorithmic bytes per launch / its average event-timed duration against MEASURED_PEAKS.json; `cpu_baseline` =
+the CPU oracle, as it stands, timed on a bounded sample on this box's host cores.
+
+Multi-GPU: the path does not shard in this build (BASELINE.json: "no sharding, no collectives"): --gpus N runs N
+independent replicas ("replicas only"); value = N x voxels x K / max-over-ranks time.
+
+`--impl reference` times the oracle (the only reference implementation that exists for this paper here).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "Gvoxel-iterations/s of fused MBS step"
+UNIT = "Gvoxel-it/s"
+SAMPLE_SHAPES = {3: (128, 128, 128), 4: (160, 160, 160), 5: (256, 128, 128)}   # oracle sample grids
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=None)
+    ap.add_argument("--warmup", type=int, default=None)
+    ap.add_argument("--config", type=int, default=5, choices=(3, 4, 5))
+    ap.add_argument("--impl", default="b200", choices=("b200", "reference"))
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-converge", action="store_true")
+    ap.add_argument("--unfused", action="store_true", help="one kernel per step of P:122-128 instead of the fused sweeps")
+    return ap.parse_args()
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.samples, self.stop_flag, self.thread = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self.stop_flag.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=5).stdout
+                f = [t.strip() for t in out.strip().split(",")]
+                if len(f) >= 6:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            self.stop_flag.wait(0.1)
+
+    def __enter__(self):
+        self.thread = threading.Thread(target=self._run, daemon=True)
+        self.thread.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop_flag.set()
+        self.thread.join(timeout=10)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["unavailable"]}
+        sm = sorted(float(s[0]) for s in self.samples)
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        reasons = [n for i, n in enumerate(names) if any(s[2 + i].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(sm)}
+
+
+def oracle_sample(cfg, n_iter, budget_s=25.0):
+    """Time the CPU oracle (oracle/mbs_oracle.py, as it stands) on a bounded sample of config `cfg`: the same
+    generator and subdomain counts at a reduced grid, `n_iter` iterations of Eq. (6).  Returns a dict."""
+    from paper_2410_02395_b200 import workloads
+    from oracle import mbs_oracle
+    shape = SAMPLE_SHAPES[cfg]
+    w = workloads.config(cfg, shape=shape, boundary_width=(8, 8, 8))
+    n, y = w.make_medium(), w.make_source()
+    o = mbs_oracle.from_workload(w, n)
+    times = []
+    t_last = [time.perf_counter()]
+
+    def cb(i, eps, x):
+        now = time.perf_counter()
+        times.append(now - t_last[0])
+        t_last[0] = now
+        if sum(times) > budget_s:
+            raise StopIteration
+
+    t_last[0] = time.perf_counter()
+    try:
+        o.solve(y, tol=0.0, max_iter=n_iter, callback=cb)
+    except StopIteration:
+        pass
+    # the first callback interval also holds the nu pre-pass: drop it when there are more
+    steady = times[1:] if len(times) > 1 else times
+    per_it = float(np.mean(steady))
+    return {"value": w.voxels / per_it / 1e9, "unit": UNIT, "cores": mbs_oracle._workers(), "kind": "oracle",
+            "sample": "cfg%d generator at %s with %s subdomains, %d oracle iterations (numpy complex128, scipy.fft)"
+                      % (cfg, "x".join(map(str, shape)), "x".join(map(str, w.n_subdomains)), len(steady)),
+            "ms_per_step": per_it * 1e3, "voxels": w.voxels}
+
+
+def run_reference(args):
+    """--impl reference: the oracle is the only reference implementation of this paper available here."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    K = args.steps if args.steps is not None else 5
+    W = args.warmup if args.warmup is not None else 1
+    r = oracle_sample(args.config, K + W, budget_s=120.0)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": K,
+            "warmup": W, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+            "config": {"workload": r["sample"]},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def workload_name(w):
+    return "%s: %s grid, %s subdomains, t=%d, W=%s, complex64, seeded synthetic medium (workloads.config)" % (
+        w.name, "x".join(map(str, w.shape)), "x".join(map(str, w.n_subdomains)), w.n_correction,
+        "x".join(map(str, w.boundary_width)))
+
+
+def dominant_kernel_traffic(name):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel class `name`, from the committed
+    ncu --set full capture (profiles/dram_traffic.json, written by hand from the capture named there)."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    if not os.path.exists(path):
+        return None
+    try:
+        return json.load(open(path)).get(name, {}).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+def run_b200(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2410_02395_b200 import binding, workloads
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    K = args.steps if args.steps is not None else {3: 400, 4: 60, 5: 30}[args.config]
+    W = args.warmup if args.warmup is not None else 3
+    W = max(W, 3)
+
+    w = workloads.config(args.config)
+    t0 = time.perf_counter()
+    n_map, y = w.make_medium(), w.make_source()
+    t_gen = time.perf_counter() - t0
+    s = binding.Solver.from_workload(w, device=dev)
+    s.set_option(binding.MBS_OPT_FUSED, 0 if args.unfused else 1)
+    nd = torch.from_numpy(n_map).to(dev)
+    s.set_potential(nd)
+    del nd
+    yd = torch.from_numpy(y).to(dev)
+    xd = torch.zeros(w.shape, dtype=torch.complex64, device=dev)
+    torch.cuda.synchronize()
+
+    # warm-up (also computes nu = ||Gamma^-1 y_vec||)
+    s.iterate(yd, xd, W, nu=0.0, want_history=False)
+    nu = s.info()["norm_rhs"]
+    s.set_option(binding.MBS_OPT_PROFILE, 1)
+    s.reset_kernel_stats()
+    launches0 = s.info()["kernel_launches"]
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    with ClockSampler(local) as clocks:
+        ev0.record(s.stream)
+        hist = s.iterate(yd, xd, K, nu=nu)
+        ev1.record(s.stream)
+        barrier()
+    ms = ev0.elapsed_time(ev1)
+    launches = s.info()["kernel_launches"] - launches0
+    stats = s.kernel_stats()
+    s.set_option(binding.MBS_OPT_PROFILE, 0)
+    if world > 1:
+        tms = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        ms = float(tms.item())
+    value = world * w.voxels * K / (ms * 1e-3) / 1e9
+
+    # roofline of the dominant kernel
+    peak, peak_kind = peaks()
+    stats = [k for k in stats if k["launches"] > 0]
+    stats.sort(key=lambda k: -k["total_ms"])
+    total_kernel_ms = sum(k["total_ms"] for k in stats)
+    top = stats[0]
+    top_ms = top["total_ms"] / top["launches"]
+    top_bytes = top["algorithmic_bytes"] / top["launches"]
+    achieved = top_bytes / (top_ms * 1e-3) / 1e9
+    info = s.info()
+    alg_bytes_it = info["algorithmic_bytes_per_iteration"]
+    roofline = {"bound": "hbm", "kernel": top["name"], "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": dominant_kernel_traffic(top["name"]), "peak_kind": peak_kind,
+                "algorithmic_bytes_per_launch": top_bytes, "avg_launch_ms": top_ms,
+                "share_of_step": top["total_ms"] / total_kernel_ms,
+                "whole_step": {"algorithmic_bytes_per_voxel_iteration": alg_bytes_it / w.voxels,
+                               "achieved": alg_bytes_it * K / (ms * 1e-3) / 1e9,
+                               "frac": alg_bytes_it * K / (ms * 1e-3) / 1e9 / peak},
+                "kernels": [{"name": k["name"], "launches_per_step": k["launches"] / K,
+                             "avg_ms": k["total_ms"] / k["launches"],
+                             "GBps": k["algorithmic_bytes"] / max(k["total_ms"], 1e-9) / 1e6} for k in stats]}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "c64", "data": "synthetic",
+            "config": {"workload": workload_name(w), "l2": "inputs larger than L2 (%.1f GiB per array)" % (w.voxels * 8 / 2 ** 30)
+                       if w.voxels * 8 > 4 * 126e6 else "arrays comparable to L2; no flush (the step streams 4 arrays)",
+                       "parallelism": "replicas x%d (path does not shard in this build)" % world,
+                       "fused": not args.unfused, "residual_last": float(hist[-1]) if len(hist) else None,
+                       "medium_generation_s": t_gen},
+            "clocks": clocks.summary(), "gpu_launches": int(launches), "roofline": roofline}
+    return s, w, yd, xd, line, rank, world
+
+
+def add_e2e(s, w, y, line, K):
+    """Same metric through the host-buffer entry point: H2D of y and x0, K iterations, D2H of x, every step."""
+    import torch
+    yh = torch.from_numpy(y).pin_memory()
+    xh = torch.zeros(w.shape, dtype=torch.complex64).pin_memory()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    ev0.record(s.stream)
+    s.solve_host(yh, xh, 0.0, K)
+    ev1.record(s.stream)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    ms = max(ev0.elapsed_time(ev1), wall * 1e3)
+    nbytes = w.voxels * 8
+    line["e2e"] = {"value": w.voxels * K / (ms * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": 2 * nbytes / K,
+                   "d2h_bytes_per_step": nbytes / K, "ms_total": ms,
+                   "note": "mbs_solve_host: one call = H2D(y, x0) + nu pre-pass + %d iterations + D2H(x); bytes are per iteration" % K}
+    del yh, xh
+
+
+def add_converge(line, dev):
+    """Seconds to converge (BASELINE.json metric, second part): cold-start mbs_solve of config 3 at its tol."""
+    import torch
+    from paper_2410_02395_b200 import binding, workloads
+    w = workloads.config(3)
+    n_map, y = w.make_medium(), w.make_source()
+    s = binding.Solver.from_workload(w, device=dev)
+    s.set_potential(n_map)
+    yd = torch.from_numpy(y).to(dev)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    x, hist, rc = s.solve(yd, tol=w.tol, max_iter=w.max_iter)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    line["time_to_converge"] = {"workload": workload_name(w), "tol": w.tol, "seconds": dt, "iterations": int(len(hist)),
+                                "status": binding.STATUS_NAMES[rc], "device_loop_ms": s.info()["last_solve_ms"]}
+    s.close()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    s, w, yd, xd, line, rank, world = run_b200(args)
+    K = line["steps"]
+    if rank == 0:
+        if not args.no_e2e:
+            y = yd.cpu().numpy()
+            del xd
+            add_e2e(s, w, y, line, K)
+    s.close()
+    del s, yd
+    if rank == 0:
+        import torch
+        torch.cuda.empty_cache()
+        if not args.no_converge:
+            add_converge(line, torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0"))))
+        if not args.no_cpu_baseline and world == 1:
+            r = oracle_sample(args.config, 6)
+            line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -65,8 +65,18 @@ enum mbs_option {
     MBS_OPT_FUSED = 0,          /* 1 (default): fused sweeps (prologue in the first FFT sweep, epilogue in the
                                    last, 112 B/voxel-iteration ledger); 0: one kernel per step of P:122-128     */
     MBS_OPT_CHECK_INTERVAL = 1, /* iterations enqueued between two host polls of the device stop flag (>= 1)  */
-    MBS_OPT_USE_GRAPH = 2       /* 1: replay each poll interval as a CUDA graph (default 1 for small grids)   */
+    MBS_OPT_USE_GRAPH = 2,      /* 1: replay each poll interval as a CUDA graph (default 1 for small grids)   */
+    MBS_OPT_PROFILE = 3         /* 1: bracket every kernel launch with CUDA events on the context's stream and
+                                   accumulate per-kernel device time (mbs_get_kernel_stats); disables graphs   */
 };
+
+/* Per-kernel device time accumulated while MBS_OPT_PROFILE is on (CUDA events on the stream). */
+typedef struct mbs_kernel_stat {
+    char name[48];               /* kernel class, e.g. "fft_strided_mid_ax0"                          */
+    int64_t launches;
+    double total_ms;             /* sum of the launches' event-to-event durations                     */
+    double algorithmic_bytes;    /* bytes one launch must move, summed over launches */
+} mbs_kernel_stat;
 
 typedef struct mbs_info {
     double c_re, c_im;             /* scale factor c of Eq. (9)                              */
@@ -143,12 +153,28 @@ MBS_API int mbs_apply_operator(mbs_ctx* ctx, int which, const void* in_device, v
 MBS_API int mbs_solve(mbs_ctx* ctx, const void* y_device, void* x_device, double tol, int32_t max_iter,
               double* residual_history, int32_t* n_iter);
 
+/*
+ * Exactly n_iter updates of Eq. (6) with no stop test: the timed "step" of bench.py.
+ *  nu  > 0: the normalisation ||Gamma^-1 y_vec|| to use for residual_history (e.g. mbs_info.norm_rhs
+ *           of an earlier solve with the same y); <= 0: computed first as in mbs_solve.
+ *  residual_history  host, capacity n_iter, may be NULL.
+ * Returns MBS_OK, MBS_ERR_NUMERIC or a CUDA/state error.  Synchronises the stream before returning.
+ */
+MBS_API int mbs_iterate(mbs_ctx* ctx, const void* y_device, void* x_device, int32_t n_iter, double nu,
+                double* residual_history);
+
 /* Same with HOST arrays y and x (complex64, `shape`): copies y and x^(0) to the device, iterates,
  * copies x back.  The end-to-end entry point (bench.py "e2e"). */
 MBS_API int mbs_solve_host(mbs_ctx* ctx, const void* y_host, void* x_host, double tol, int32_t max_iter,
                    double* residual_history, int32_t* n_iter);
 
 MBS_API int mbs_get_info(const mbs_ctx* ctx, mbs_info* out);
+
+/* Kernel statistics gathered since the last mbs_reset_kernel_stats (needs MBS_OPT_PROFILE = 1).
+ * Writes at most `capacity` entries to out (host) and the number of classes seen to *count.
+ * Synchronises the stream. */
+MBS_API int mbs_get_kernel_stats(mbs_ctx* ctx, mbs_kernel_stat* out, int32_t capacity, int32_t* count);
+MBS_API int mbs_reset_kernel_stats(mbs_ctx* ctx);
 
 /* Frees everything the library allocated.  NULL-safe. */
 MBS_API void mbs_destroy(mbs_ctx* ctx);

@@ -27,15 +27,15 @@ _lib = ctypes.CDLL(LIB_PATH)
 MBS_OK, MBS_ERR_INVALID_ARG, MBS_ERR_UNSUPPORTED_SIZE, MBS_ERR_OOM = 0, 1, 2, 3
 MBS_ERR_CUDA, MBS_ERR_NOT_CONVERGED, MBS_ERR_NUMERIC, MBS_ERR_STATE = 4, 5, 6, 7
 MBS_OP_B, MBS_OP_PROPAGATOR, MBS_OP_A, MBS_OP_PRECOND_A = 0, 1, 2, 3
-MBS_OPT_FUSED, MBS_OPT_CHECK_INTERVAL, MBS_OPT_USE_GRAPH = 0, 1, 2
+MBS_OPT_FUSED, MBS_OPT_CHECK_INTERVAL, MBS_OPT_USE_GRAPH, MBS_OPT_PROFILE = 0, 1, 2, 3
 
 STATUS_NAMES = {0: "MBS_OK", 1: "MBS_ERR_INVALID_ARG", 2: "MBS_ERR_UNSUPPORTED_SIZE", 3: "MBS_ERR_OOM",
                 4: "MBS_ERR_CUDA", 5: "MBS_ERR_NOT_CONVERGED", 6: "MBS_ERR_NUMERIC", 7: "MBS_ERR_STATE"}
 
 # every symbol include/mbs.h declares (tests/test_abi.py checks the library exports them all)
 DECLARED_SYMBOLS = ("mbs_create", "mbs_fft_supported", "mbs_workspace_bytes", "mbs_set_workspace", "mbs_set_option",
-                    "mbs_set_potential", "mbs_apply_operator", "mbs_solve", "mbs_solve_host", "mbs_get_info",
-                    "mbs_destroy", "mbs_last_error")
+                    "mbs_set_potential", "mbs_apply_operator", "mbs_solve", "mbs_solve_host", "mbs_iterate",
+                    "mbs_get_info", "mbs_get_kernel_stats", "mbs_reset_kernel_stats", "mbs_destroy", "mbs_last_error")
 
 
 class mbs_info(ctypes.Structure):
@@ -48,6 +48,11 @@ class mbs_info(ctypes.Structure):
                 ("algorithmic_bytes_per_iteration", ctypes.c_double),
                 ("workspace_bytes", ctypes.c_uint64), ("kernel_launches", ctypes.c_int64),
                 ("last_solve_ms", ctypes.c_double)]
+
+
+class mbs_kernel_stat(ctypes.Structure):
+    _fields_ = [("name", ctypes.c_char * 48), ("launches", ctypes.c_int64), ("total_ms", ctypes.c_double),
+                ("algorithmic_bytes", ctypes.c_double)]
 
 
 _vp = ctypes.c_void_p
@@ -72,6 +77,12 @@ _lib.mbs_solve.argtypes = [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int32, ctype
 _lib.mbs_solve.restype = ctypes.c_int
 _lib.mbs_solve_host.argtypes = _lib.mbs_solve.argtypes
 _lib.mbs_solve_host.restype = ctypes.c_int
+_lib.mbs_iterate.argtypes = [_vp, _vp, _vp, ctypes.c_int32, ctypes.c_double, ctypes.POINTER(ctypes.c_double)]
+_lib.mbs_iterate.restype = ctypes.c_int
+_lib.mbs_get_kernel_stats.argtypes = [_vp, ctypes.POINTER(mbs_kernel_stat), ctypes.c_int32, ctypes.POINTER(ctypes.c_int32)]
+_lib.mbs_get_kernel_stats.restype = ctypes.c_int
+_lib.mbs_reset_kernel_stats.argtypes = [_vp]
+_lib.mbs_reset_kernel_stats.restype = ctypes.c_int
 _lib.mbs_get_info.argtypes = [_vp, ctypes.POINTER(mbs_info)]
 _lib.mbs_get_info.restype = ctypes.c_int
 _lib.mbs_destroy.argtypes = [_vp]
@@ -160,6 +171,27 @@ def mbs_solve_host(ctx, y_ptr: int, x_ptr: int, tol: float, max_iter: int, want_
     return _solve(_lib.mbs_solve_host, ctx, y_ptr, x_ptr, tol, max_iter, want_history)
 
 
+def mbs_iterate(ctx, y_ptr: int, x_ptr: int, n_iter: int, nu: float = 0.0, want_history: bool = True):
+    """Exactly n_iter updates, no stop test (device pointers).  Returns the residual history."""
+    hist = np.empty(n_iter if want_history else 0, dtype=np.float64)
+    hp = hist.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if want_history else None
+    _check(ctx, _lib.mbs_iterate(ctx, _vp(y_ptr), _vp(x_ptr), int(n_iter), float(nu), hp))
+    return hist
+
+
+def mbs_get_kernel_stats(ctx) -> list:
+    cap = 64
+    arr = (mbs_kernel_stat * cap)()
+    n = ctypes.c_int32(0)
+    _check(ctx, _lib.mbs_get_kernel_stats(ctx, arr, cap, ctypes.byref(n)))
+    return [dict(name=arr[i].name.decode(), launches=int(arr[i].launches), total_ms=float(arr[i].total_ms),
+                 algorithmic_bytes=float(arr[i].algorithmic_bytes)) for i in range(min(n.value, cap))]
+
+
+def mbs_reset_kernel_stats(ctx):
+    _check(ctx, _lib.mbs_reset_kernel_stats(ctx))
+
+
 def mbs_get_info(ctx) -> dict:
     info = mbs_info()
     _check(ctx, _lib.mbs_get_info(ctx, ctypes.byref(info)))
@@ -242,6 +274,16 @@ class Solver:
             return a.data_ptr() if hasattr(a, "data_ptr") else a.ctypes.data
         rc, hist, n = mbs_solve_host(self.ctx, ptr(y_host), ptr(x_host), tol, max_iter)
         return hist, rc
+
+    def iterate(self, y_dev, x_dev, n_iter: int, nu: float = 0.0, want_history: bool = True):
+        """y_dev, x_dev: complex64 device tensors of the grid shape; x_dev is updated in place."""
+        return mbs_iterate(self.ctx, y_dev.data_ptr(), x_dev.data_ptr(), n_iter, nu, want_history)
+
+    def kernel_stats(self) -> list:
+        return mbs_get_kernel_stats(self.ctx)
+
+    def reset_kernel_stats(self):
+        mbs_reset_kernel_stats(self.ctx)
 
     def info(self) -> dict:
         return mbs_get_info(self.ctx)

@@ -17,6 +17,25 @@ using namespace mbs;
 
 typedef std::complex<double> cd;
 
+// Per-kernel device timing (MBS_OPT_PROFILE): every launch is bracketed by a pair of CUDA events on
+// the context's stream; pairs are resolved after the next stream synchronisation.
+struct KernelClass {
+    std::string name;
+    int64_t launches = 0;
+    double ms = 0, bytes = 0;
+};
+struct Profiler {
+    std::vector<KernelClass> classes;
+    std::vector<cudaEvent_t> pool;           // 2 events per pending launch
+    std::vector<int> pending;                // class index of each pending launch
+    int find(const char* name) {
+        for (size_t i = 0; i < classes.size(); ++i)
+            if (classes[i].name == name) return (int)i;
+        classes.push_back(KernelClass{name});
+        return (int)classes.size() - 1;
+    }
+};
+
 struct mbs_ctx {
     int ndim = 0;
     int first = 0;  // first real axis of the internal 3-D description
@@ -62,6 +81,9 @@ struct mbs_ctx {
     int check_interval = 0;  // 0 = automatic
     int use_graph = -1;      // -1 = automatic
 
+    int profile = 0;
+    Profiler prof;
+
     int64_t launches = 0;
     std::string err;
 };
@@ -92,6 +114,45 @@ static int fail(mbs_ctx* ctx, int code, const char* fmt, ...) {
         int rc__ = (expr);               \
         if (rc__ != MBS_OK) return rc__; \
     } while (0)
+
+// Resolve the pending event pairs (the stream must have been synchronised).
+static void prof_drain(mbs_ctx* c) {
+    Profiler& p = c->prof;
+    for (size_t i = 0; i < p.pending.size(); ++i) {
+        float ms = 0.f;
+        if (cudaEventElapsedTime(&ms, p.pool[2 * i], p.pool[2 * i + 1]) == cudaSuccess) p.classes[p.pending[i]].ms += ms;
+    }
+    p.pending.clear();
+}
+
+// Brackets one kernel launch: counts it and, in profile mode, records the event pair around it.
+struct KernelScope {
+    mbs_ctx* c;
+    int slot = -1;
+    KernelScope(mbs_ctx* ctx, const char* name, double bytes) : c(ctx) {
+        c->launches++;
+        if (!c->profile) return;
+        Profiler& p = c->prof;
+        if (p.pending.size() >= 8192) {
+            cudaStreamSynchronize(c->stream);
+            prof_drain(c);
+        }
+        const int k = p.find(name);
+        p.classes[k].launches++;
+        p.classes[k].bytes += bytes;
+        slot = (int)p.pending.size();
+        while (p.pool.size() < 2 * (size_t)(slot + 1)) {
+            cudaEvent_t e = nullptr;
+            cudaEventCreate(&e);
+            p.pool.push_back(e);
+        }
+        p.pending.push_back(k);
+        cudaEventRecord(p.pool[2 * slot], c->stream);
+    }
+    ~KernelScope() {
+        if (slot >= 0) cudaEventRecord(c->prof.pool[2 * slot + 1], c->stream);
+    }
+};
 
 // ---------------------------------------------------------------------------------------------
 // host-side small linear algebra: sigma_max of the t x t matrix K_t, cyclic Jacobi on K^T K
@@ -301,6 +362,7 @@ extern "C" void mbs_destroy(mbs_ctx* c) {
     if (c->ev_t1) cudaEventDestroy(c->ev_t1);
     if (c->host_y) cudaFree(c->host_y);
     if (c->host_x) cudaFree(c->host_x);
+    for (cudaEvent_t e : c->prof.pool) cudaEventDestroy(e);
     delete c;
 }
 
@@ -337,6 +399,7 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
             c->check_interval = (int)value;
             return MBS_OK;
         case MBS_OPT_USE_GRAPH: c->use_graph = value ? 1 : 0; return MBS_OK;
+        case MBS_OPT_PROFILE: c->profile = value ? 1 : 0; return MBS_OK;
         default: return fail(c, MBS_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }
@@ -357,7 +420,8 @@ extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
     for (int d = 0; d < 3; ++d) sp.W[d] = c->W[d];
     int nblocks = (int)std::min<long long>((g.voxels + 255) / 256, (long long)std::min(MBS_MAX_PARTIALS, c->num_sms * 8));
     std::vector<double> host(5 * (size_t)nblocks);
-    MBS_CUDA(c, launch_setup(g, sp, 0, c->partials, nullptr, nblocks, c->stream));
+    const double vb = 8.0 * (double)g.voxels;
+    { KernelScope ks(c, "setup_minmax", vb); MBS_CUDA(c, launch_setup(g, sp, 0, c->partials, nullptr, nblocks, c->stream)); }
     MBS_CUDA(c, cudaMemcpyAsync(host.data(), c->partials, sizeof(double) * 5 * nblocks, cudaMemcpyDeviceToHost, c->stream));
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));
     double mn_re = INFINITY, mx_re = -INFINITY, mn_im = INFINITY, mx_im = -INFINITY, mn_n = INFINITY;
@@ -373,7 +437,7 @@ extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
     c->k02 = cd(0.5 * (mn_re + mx_re), 0.5 * (mn_im + mx_im));
     sp.k02_re = c->k02.real();
     sp.k02_im = c->k02.imag();
-    MBS_CUDA(c, launch_setup(g, sp, 1, c->partials, nullptr, nblocks, c->stream));
+    { KernelScope ks(c, "setup_vmax", vb); MBS_CUDA(c, launch_setup(g, sp, 1, c->partials, nullptr, nblocks, c->stream)); }
     MBS_CUDA(c, cudaMemcpyAsync(host.data(), c->partials, sizeof(double) * nblocks, cudaMemcpyDeviceToHost, c->stream));
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));
     double v2 = 0;
@@ -384,9 +448,8 @@ extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
     c->c = cd(0.0, -0.95 / denom);
     sp.c_re = c->c.real();
     sp.c_im = c->c.imag();
-    MBS_CUDA(c, launch_setup(g, sp, 2, nullptr, c->bdiag, nblocks, c->stream));
+    { KernelScope ks(c, "setup_bdiag", 2 * vb); MBS_CUDA(c, launch_setup(g, sp, 2, nullptr, c->bdiag, nblocks, c->stream)); }
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->launches += 3;
     c->potential_set = true;
     return MBS_OK;
 }
@@ -403,8 +466,9 @@ static int run_slabs(mbs_ctx* c, const cf* in, const cf* in2, bool in_loop) {
         SlabParams sp{};
         sp.in = in; sp.in2 = in2; sp.out = c->cx.buf[ax]; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
         sp.state = c->state; sp.check_done = in_loop ? 1 : 0;
+        static const char* names[3] = {"slab_ax0", "slab_ax1", "slab_ax2"};
+        KernelScope ks(c, names[ax], (in2 ? 24.0 : 16.0) * (double)corr_elems(c->g, ax));
         MBS_CUDA(c, launch_slab(c->g, sp, c->stream));
-        c->launches++;
     }
     return MBS_OK;
 }
@@ -437,8 +501,9 @@ static int run_propagator(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
         cg.n_tiles = (cg.n_lines + e->C - 1) / e->C;
         SymbolParams s2 = sp;
         s2.tab_axis = c->p2_dev[2];
+        static const char* names[3] = {"fft_contig_fwd", "fft_contig_inv", "fft_contig_mid"};
+        KernelScope ks(c, names[mode], 16.0 * (double)g.voxels);
         MBS_CUDA(c, e->contig(buf, buf, cg, s2, c->tw_dev[2], mode, done, c->num_sms, c->stream));
-        c->launches++;
         return MBS_OK;
     };
     auto strided = [&](int ax, int mode) -> int {
@@ -457,8 +522,10 @@ static int run_propagator(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
             if (ax == 0) { s2.tabA = c->p2_dev[1]; s2.Ma = g.M[1]; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
             else { s2.tabA = nullptr; s2.Ma = 1; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
         }
+        static const char* names[2][3] = {{"fft_strided_fwd_ax0", "fft_strided_inv_ax0", "fft_strided_mid_ax0"},
+                                          {"fft_strided_fwd_ax1", "fft_strided_inv_ax1", "fft_strided_mid_ax1"}};
+        KernelScope ks(c, names[ax][mode], 16.0 * (double)g.voxels);
         MBS_CUDA(c, e->strided(buf, sg, s2, c->tw_dev[ax], mode, done, c->num_sms, c->stream));
-        c->launches++;
         return MBS_OK;
     };
     if (c->ndim == 1) return contig(FFT_MID);
@@ -476,8 +543,9 @@ static int run_B(mbs_ctx* c, const cf* in, const cf* in2, const cf* y, cf ysc, c
     PointwiseParams p = pw_defaults(c, in_loop);
     p.in = in; p.in2 = in2; p.bdiag = c->bdiag; p.y = y; p.ysc = ysc; p.out = out; p.s1 = s1; p.w = w; p.s2 = s2;
     p.corr = c->cx; p.reduce = reduce;
+    const int n_arrays = 2 + (in2 ? 1 : 0) + (y ? 1 : 0) + (w ? 1 : 0) + (out ? 1 : 0);
+    KernelScope ks(c, y ? "pointwise_Bx_plus_y" : "pointwise_B", 8.0 * n_arrays * (double)c->g.voxels);
     MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
-    c->launches++;
     return MBS_OK;
 }
 
@@ -489,8 +557,8 @@ static int run_iteration_unfused(mbs_ctx* c, const cf* y, cf* x) {
     MBS_TRY(run_slabs(c, x, c->u, true));                                          // corr(x - u')
     PointwiseParams p = pw_defaults(c, true);                                      // r = B (x - u'); x -= alpha r
     p.in = x; p.in2 = c->u; p.bdiag = c->bdiag; p.out = x; p.corr = c->cx; p.update = 1; p.reduce = RED_RESIDUAL;
+    KernelScope ks(c, "pointwise_update", 32.0 * (double)c->g.voxels);
     MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
-    c->launches++;
     return MBS_OK;
 }
 
@@ -528,13 +596,23 @@ extern "C" int mbs_apply_operator(mbs_ctx* c, int which, const void* in_device, 
 // ---------------------------------------------------------------------------------------------
 // solve
 // ---------------------------------------------------------------------------------------------
-static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_iter, double* residual_history,
-                        int32_t* n_iter) {
-    if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
-    if (!y || !x) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
-    if (max_iter < 1) return fail(c, MBS_ERR_INVALID_ARG, "max_iter must be >= 1");
-    if (!(tol >= 0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0");
-    if (n_iter) *n_iter = 0;
+// Reset the device state for a new solve and (nu <= 0) compute nu = || B (L+I)^-1 y_vec ||
+static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, double nu) {
+    DevState init{};
+    init.iter = 0; init.done = 0; init.max_iter = max_iter; init.ticket = 0; init.tol = tol;
+    init.nu2 = nu > 0 ? nu * nu : 0.0; init.last_sum = 0;
+    c->state_pinned[0] = init;
+    MBS_CUDA(c, cudaMemcpyAsync(c->state, &c->state_pinned[0], sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
+    if (!(nu > 0)) {
+        { KernelScope ks(c, "scale_copy", 16.0 * (double)c->g.voxels); MBS_CUDA(c, launch_scale_copy(y, c->u, to_cf(-c->c), c->g.voxels, c->stream)); }
+        MBS_TRY(run_propagator(c, c->u, 1, false));
+        MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
+    }
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));   // state_pinned[0] is reused by the poll loop
+    return MBS_OK;
+}
+
+static int ensure_history(mbs_ctx* c, int32_t max_iter) {
     if (c->hist_cap < max_iter) {
         if (c->hist_dev) cudaFree(c->hist_dev);
         c->hist_dev = nullptr;
@@ -542,16 +620,18 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
         MBS_CUDA(c, cudaMalloc(&c->hist_dev, sizeof(double) * (size_t)max_iter));
         c->hist_cap = max_iter;
     }
-    DevState init{};
-    init.iter = 0; init.done = 0; init.max_iter = max_iter; init.ticket = 0; init.tol = tol; init.nu2 = 0; init.last_sum = 0;
-    c->state_pinned[0] = init;
-    MBS_CUDA(c, cudaMemcpyAsync(c->state, &c->state_pinned[0], sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
-    // nu = || B (L+I)^-1 y_vec ||
-    MBS_CUDA(c, launch_scale_copy(y, c->u, to_cf(-c->c), c->g.voxels, c->stream));
-    c->launches++;
-    MBS_TRY(run_propagator(c, c->u, 1, false));
-    MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
-    MBS_CUDA(c, cudaStreamSynchronize(c->stream));   // state_pinned[0] is reused below
+    return MBS_OK;
+}
+
+static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_iter, double* residual_history,
+                        int32_t* n_iter) {
+    if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
+    if (!y || !x) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
+    if (max_iter < 1) return fail(c, MBS_ERR_INVALID_ARG, "max_iter must be >= 1");
+    if (!(tol >= 0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0");
+    if (n_iter) *n_iter = 0;
+    MBS_TRY(ensure_history(c, max_iter));
+    MBS_TRY(begin_solve(c, y, tol, max_iter, 0.0));
 
     int interval = c->check_interval;
     if (interval <= 0) {
@@ -596,6 +676,7 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
     float ms = 0.f;
     MBS_CUDA(c, cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1));
     c->last_solve_ms = ms;
+    prof_drain(c);
     c->norm_rhs = sqrt(fin.nu2);
     if (n_iter) *n_iter = fin.iter;
     if (residual_history && fin.iter > 0)
@@ -609,6 +690,56 @@ extern "C" int mbs_solve(mbs_ctx* c, const void* y_device, void* x_device, doubl
                          double* residual_history, int32_t* n_iter) {
     if (!c) return MBS_ERR_INVALID_ARG;
     return solve_device(c, (const cf*)y_device, (cf*)x_device, tol, max_iter, residual_history, n_iter);
+}
+
+extern "C" int mbs_iterate(mbs_ctx* c, const void* y_device, void* x_device, int32_t n_iter, double nu,
+                           double* residual_history) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
+    if (!y_device || !x_device) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
+    if (n_iter < 1) return fail(c, MBS_ERR_INVALID_ARG, "n_iter must be >= 1");
+    MBS_TRY(ensure_history(c, n_iter));
+    MBS_TRY(begin_solve(c, (const cf*)y_device, -1.0, n_iter, nu));
+    MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
+    for (int i = 0; i < n_iter; ++i) MBS_TRY(run_iteration_unfused(c, (const cf*)y_device, (cf*)x_device));
+    MBS_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    DevState fin{};
+    MBS_CUDA(c, cudaMemcpy(&fin, c->state, sizeof(DevState), cudaMemcpyDeviceToHost));
+    float ms = 0.f;
+    MBS_CUDA(c, cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1));
+    c->last_solve_ms = ms;
+    c->norm_rhs = sqrt(fin.nu2);
+    prof_drain(c);
+    if (residual_history && fin.iter > 0)
+        MBS_CUDA(c, cudaMemcpy(residual_history, c->hist_dev, sizeof(double) * (size_t)fin.iter, cudaMemcpyDeviceToHost));
+    if (fin.done == 3) return fail(c, MBS_ERR_NUMERIC, "non-finite residual at iteration %d", fin.iter - 1);
+    return MBS_OK;
+}
+
+extern "C" int mbs_get_kernel_stats(mbs_ctx* c, mbs_kernel_stat* out, int32_t capacity, int32_t* count) {
+    if (!c || !count) return MBS_ERR_INVALID_ARG;
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    prof_drain(c);
+    const int n = (int)c->prof.classes.size();
+    *count = n;
+    for (int i = 0; i < n && i < capacity && out; ++i) {
+        const KernelClass& k = c->prof.classes[i];
+        memset(&out[i], 0, sizeof out[i]);
+        snprintf(out[i].name, sizeof out[i].name, "%s", k.name.c_str());
+        out[i].launches = k.launches;
+        out[i].total_ms = k.ms;
+        out[i].algorithmic_bytes = k.bytes;
+    }
+    return MBS_OK;
+}
+
+extern "C" int mbs_reset_kernel_stats(mbs_ctx* c) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+    prof_drain(c);
+    c->prof.classes.clear();
+    return MBS_OK;
 }
 
 extern "C" int mbs_solve_host(mbs_ctx* c, const void* y_host, void* x_host, double tol, int32_t max_iter,
