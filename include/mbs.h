@@ -66,6 +66,8 @@ enum mbs_option {
                                    last, 112 B/voxel-iteration ledger); 0: one kernel per step of P:122-128     */
     MBS_OPT_CHECK_INTERVAL = 1, /* iterations enqueued between two host polls of the device stop flag (>= 1)  */
     MBS_OPT_USE_GRAPH = 2,      /* 1: replay each poll interval as a CUDA graph (default 1 for small grids)   */
+    MBS_OPT_TMA = 4,            /* 1 (default): strided-axis FFT sweeps are fed by TMA box loads/stores through a
+                                   shared-memory stage ring; 0: threads load/store the tiles themselves        */
     MBS_OPT_PROFILE = 3         /* 1: bracket every kernel launch with CUDA events on the context's stream and
                                    accumulate per-kernel device time (mbs_get_kernel_stats); disables graphs   */
 };

@@ -54,6 +54,7 @@ struct mbs_ctx {
     CorrBufs cx{};  // edge corrections of the current operand
     CorrBufs ds{};  // fused path: d = x - u' at the slab voxels of the non-contiguous axes
     double* partials = nullptr;
+    unsigned char* ymask = nullptr;  // per grid row: the source row is not all zero
 
     // small library-owned device data
     DevState* state = nullptr;
@@ -77,9 +78,10 @@ struct mbs_ctx {
     std::vector<double> Kh;  // t*t
 
     // options
-    int fused = 0;
+    int fused = 1;
     int check_interval = 0;  // 0 = automatic
     int use_graph = -1;      // -1 = automatic
+    int use_tma = 1;         // TMA-fed strided sweeps
 
     int profile = 0;
     Profiler prof;
@@ -231,6 +233,7 @@ static size_t layout_workspace(mbs_ctx* c, char* base) {
     }
     c->ds.buf[2] = nullptr;
     c->partials = (double*)take(sizeof(double) * MBS_MAX_PARTIALS * 5);
+    c->ymask = (unsigned char*)take((size_t)(g.voxels / g.N[2]));
     return off;
 }
 
@@ -400,6 +403,7 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
             return MBS_OK;
         case MBS_OPT_USE_GRAPH: c->use_graph = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_PROFILE: c->profile = value ? 1 : 0; return MBS_OK;
+        case MBS_OPT_TMA: c->use_tma = value ? 1 : 0; return MBS_OK;
         default: return fail(c, MBS_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }
@@ -460,11 +464,12 @@ extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
 static cf to_cf(cd z) { return make_float2((float)z.real(), (float)z.imag()); }
 
 // edge corrections of (in - in2) into c->cx  (a2 / a7 of the scope table)
-static int run_slabs(mbs_ctx* c, const cf* in, const cf* in2, bool in_loop) {
+static int run_slabs(mbs_ctx* c, const cf* in, const cf* in2, bool in_loop, int axis_mask = 7, bool from_ds = false) {
     for (int ax = 0; ax < 3; ++ax) {
-        if (!c->cx.buf[ax]) continue;
+        if (!c->cx.buf[ax] || !((axis_mask >> ax) & 1)) continue;
         SlabParams sp{};
-        sp.in = in; sp.in2 = in2; sp.out = c->cx.buf[ax]; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
+        sp.in = from_ds ? c->ds.buf[ax] : in; sp.in2 = in2; sp.out = c->cx.buf[ax]; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
+        sp.compact_in = from_ds ? 1 : 0;
         sp.state = c->state; sp.check_done = in_loop ? 1 : 0;
         static const char* names[3] = {"slab_ax0", "slab_ax1", "slab_ax2"};
         KernelScope ks(c, names[ax], (in2 ? 24.0 : 16.0) * (double)corr_elems(c->g, ax));
@@ -482,8 +487,7 @@ static PointwiseParams pw_defaults(mbs_ctx* c, bool in_loop) {
     return p;
 }
 
-// (L+I)^-1 (inverse = 1) or (L+I) (inverse = 0) in place on buf  (a3-a5 of the scope table)
-static int run_propagator(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
+static SymbolParams make_symbol(const mbs_ctx* c, int inverse) {
     const GridDesc& g = c->g;
     SymbolParams sp{};
     const cd ck = c->c * c->k02;
@@ -491,49 +495,66 @@ static int run_propagator(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
     sp.B0 = (float)ck.imag();
     sp.cr = (float)c->c.real();
     sp.ci = (float)c->c.imag();
-    sp.scale = (float)(1.0 / ((double)g.M[0] * g.M[1] * g.M[2]));
+    sp.scale = (float)(1.0 / ((double)g.M[0] * g.M[1] * g.M[2]));   // 1/M of the inverse transforms (R9)
     sp.inverse = inverse;
-    const int* done = in_loop ? &c->state->done : nullptr;
-    auto contig = [&](int mode) -> int {
-        ContigGeom cg{};
-        const FftEntry* e = c->fft[2];
-        cg.n_lines = g.voxels / g.M[2];
-        cg.n_tiles = (cg.n_lines + e->C - 1) / e->C;
-        SymbolParams s2 = sp;
-        s2.tab_axis = c->p2_dev[2];
-        static const char* names[3] = {"fft_contig_fwd", "fft_contig_inv", "fft_contig_mid"};
-        KernelScope ks(c, names[mode], 16.0 * (double)g.voxels);
-        MBS_CUDA(c, e->contig(buf, buf, cg, s2, c->tw_dev[2], mode, done, c->num_sms, c->stream));
-        return MBS_OK;
-    };
-    auto strided = [&](int ax, int mode) -> int {
-        const FftEntry* e = c->fft[ax];
-        StridedGeom sg{};
-        long long inner = 1, outer = 1;
-        for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
-        for (int d = 0; d < ax; ++d) outer *= g.N[d];
-        sg.stride = inner; sg.outer_stride = (long long)g.N[ax] * inner; sg.n_outer = (int)outer; sg.n_seg = g.S[ax];
-        sg.inner = (int)inner; sg.tiles_inner = (int)((inner + e->C - 1) / e->C);
-        sg.n_tiles = outer * g.S[ax] * sg.tiles_inner;
-        SymbolParams s2 = sp;
-        s2.tab_axis = c->p2_dev[ax];
-        if (mode == FFT_MID) {
-            // line-invariant part of |p|^2 from the axes after `ax`
-            if (ax == 0) { s2.tabA = c->p2_dev[1]; s2.Ma = g.M[1]; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
-            else { s2.tabA = nullptr; s2.Ma = 1; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
-        }
-        static const char* names[2][3] = {{"fft_strided_fwd_ax0", "fft_strided_inv_ax0", "fft_strided_mid_ax0"},
-                                          {"fft_strided_fwd_ax1", "fft_strided_inv_ax1", "fft_strided_mid_ax1"}};
-        KernelScope ks(c, names[ax][mode], 16.0 * (double)g.voxels);
-        MBS_CUDA(c, e->strided(buf, sg, s2, c->tw_dev[ax], mode, done, c->num_sms, c->stream));
-        return MBS_OK;
-    };
-    if (c->ndim == 1) return contig(FFT_MID);
-    MBS_TRY(contig(FFT_FWD));
-    if (c->ndim == 3) MBS_TRY(strided(1, FFT_FWD));
-    MBS_TRY(strided(c->first, FFT_MID));
-    if (c->ndim == 3) MBS_TRY(strided(1, FFT_INV));
-    return contig(FFT_INV);
+    return sp;
+}
+
+// FFT sweep along the contiguous axis, in place on buf
+static int run_fft_contig(mbs_ctx* c, cf* buf, int mode, int inverse, bool in_loop) {
+    const GridDesc& g = c->g;
+    ContigGeom cg{};
+    const FftEntry* e = c->fft[2];
+    cg.n_lines = g.voxels / g.M[2];
+    cg.n_tiles = (cg.n_lines + e->C - 1) / e->C;
+    SymbolParams s2 = make_symbol(c, inverse);
+    s2.tab_axis = c->p2_dev[2];
+    static const char* names[3] = {"fft_contig_fwd", "fft_contig_inv", "fft_contig_mid"};
+    KernelScope ks(c, names[mode], 16.0 * (double)g.voxels);
+    MBS_CUDA(c, e->contig(buf, buf, cg, s2, c->tw_dev[2], mode, in_loop ? &c->state->done : nullptr, c->num_sms, c->stream));
+    return MBS_OK;
+}
+
+// FFT sweep along strided axis ax (0 or 1), in place on buf
+static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, bool in_loop) {
+    const GridDesc& g = c->g;
+    const FftEntry* e = c->fft[ax];
+    StridedGeom sg{};
+    long long inner = 1, outer = 1;
+    for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
+    for (int d = 0; d < ax; ++d) outer *= g.N[d];
+    sg.stride = inner; sg.outer_stride = (long long)g.N[ax] * inner; sg.n_outer = (int)outer; sg.n_seg = g.S[ax];
+    sg.inner = (int)inner; sg.tiles_inner = (int)((inner + e->C - 1) / e->C);
+    sg.n_tiles = outer * g.S[ax] * sg.tiles_inner;
+    SymbolParams s2 = make_symbol(c, inverse);
+    s2.tab_axis = c->p2_dev[ax];
+    if (mode == FFT_MID) {
+        // line-invariant part of |p|^2 from the axes after `ax`
+        if (ax == 0) { s2.tabA = c->p2_dev[1]; s2.Ma = g.M[1]; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
+        else { s2.tabA = nullptr; s2.Ma = 1; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
+    }
+    static const char* names[2][3] = {{"fft_strided_fwd_ax0", "fft_strided_inv_ax0", "fft_strided_mid_ax0"},
+                                      {"fft_strided_fwd_ax1", "fft_strided_inv_ax1", "fft_strided_mid_ax1"}};
+    KernelScope ks(c, names[ax][mode], 16.0 * (double)g.voxels);
+    MBS_CUDA(c, e->strided(buf, sg, s2, c->tw_dev[ax], mode, in_loop ? &c->state->done : nullptr, c->num_sms, c->use_tma,
+                           c->stream));
+    return MBS_OK;
+}
+
+// the sweeps between the first and the last one: strided forward, kernel multiply, strided inverse (a3-a5)
+static int run_middle_sweeps(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
+    if (c->ndim == 3) MBS_TRY(run_fft_strided(c, buf, 1, FFT_FWD, inverse, in_loop));
+    MBS_TRY(run_fft_strided(c, buf, c->first, FFT_MID, inverse, in_loop));
+    if (c->ndim == 3) MBS_TRY(run_fft_strided(c, buf, 1, FFT_INV, inverse, in_loop));
+    return MBS_OK;
+}
+
+// (L+I)^-1 (inverse = 1) or (L+I) (inverse = 0) in place on buf  (a3-a5 of the scope table)
+static int run_propagator(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
+    if (c->ndim == 1) return run_fft_contig(c, buf, FFT_MID, inverse, in_loop);
+    MBS_TRY(run_fft_contig(c, buf, FFT_FWD, inverse, in_loop));
+    MBS_TRY(run_middle_sweeps(c, buf, inverse, in_loop));
+    return run_fft_contig(c, buf, FFT_INV, inverse, in_loop);
 }
 
 // out = s1 * [B_diag (in - in2) + ysc*y - corr(in - in2)] + s2*w
@@ -560,6 +581,64 @@ static int run_iteration_unfused(mbs_ctx* c, const cf* y, cf* x) {
     KernelScope ks(c, "pointwise_update", 32.0 * (double)c->g.voxels);
     MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
     return MBS_OK;
+}
+
+// The fused path needs whole grid rows inside one tile of the contiguous-axis kernel.
+static bool fused_available(const mbs_ctx* c) { return c->fft[2]->C % c->g.S[2] == 0; }
+
+// one iteration of Eq. (6), fused sweeps (112 B/voxel ledger of DESIGN.md section 5)
+static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
+    const GridDesc& g = c->g;
+    const FftEntry* e = c->fft[2];
+    const int e0 = g.a[0] > 0, e1 = g.a[1] > 0;
+    const int* done = &c->state->done;
+    FusedParams p{};
+    p.x = x; p.bdiag = c->bdiag; p.y = y; p.ymask = c->ymask; p.ysc = to_cf(-c->c); p.u = c->u;
+    p.N1 = g.N[1]; p.N2 = g.N[2]; p.S2 = g.S[2]; p.a2 = g.a[2]; p.per2 = g.per[2]; p.t = g.t;
+    p.e0 = e0; p.e1 = e1; p.M0 = g.M[0]; p.M1 = g.M[1]; p.S1 = g.S[1];
+    p.cx0 = c->cx.buf[0]; p.cx1 = c->cx.buf[1]; p.ds0 = c->ds.buf[0]; p.ds1 = c->ds.buf[1];
+    p.Kh = c->Kh_dev; p.c = to_cf(c->c); p.alpha = (float)c->alpha;
+    p.sp = make_symbol(c, 1); p.sp.tab_axis = c->p2_dev[2];
+    p.n_lines = g.voxels / g.M[2];
+    p.n_tiles = (p.n_lines + e->C - 1) / e->C;
+    p.partials = c->partials; p.state = c->state; p.hist = c->hist_dev; p.reduce_mode = RED_RESIDUAL;
+    const double vb = 8.0 * (double)g.voxels;
+    if (c->ndim == 1) {
+        p.slot0 = 0; p.finish = 1;
+        p.n_total = e->fused_blocks(FUSED_1D, g.t, p.n_tiles, c->num_sms);
+        KernelScope ks(c, "fused_1d", 4 * vb);
+        MBS_CUDA(c, e->fused(p, c->tw_dev[2], FUSED_1D, done, c->num_sms, c->stream));
+        return MBS_OK;
+    }
+    const int mask01 = (e0 ? 1 : 0) | (e1 ? 2 : 0);
+    if (mask01) MBS_TRY(run_slabs(c, x, nullptr, true, mask01));                      // corr_0(x), corr_1(x)
+    {
+        KernelScope ks(c, "fused_sweep1", 4 * vb);                                    // reads x, B_diag, y; writes u
+        MBS_CUDA(c, e->fused(p, c->tw_dev[2], FUSED_S1, done, c->num_sms, c->stream));
+    }
+    MBS_TRY(run_middle_sweeps(c, c->u, 1, true));
+    const int nb5 = e->fused_blocks(FUSED_S5, g.t, p.n_tiles, c->num_sms);
+    if (nb5 < 1) return fail(c, MBS_ERR_CUDA, "fused sweep: occupancy query failed");
+    p.slot0 = 0; p.n_total = nb5; p.finish = mask01 ? 0 : 1;
+    {
+        KernelScope ks(c, "fused_sweep5", 4 * vb);                                    // reads u, x, B_diag; writes x
+        MBS_CUDA(c, e->fused(p, c->tw_dev[2], FUSED_S5, done, c->num_sms, c->stream));
+    }
+    if (mask01) {
+        MBS_TRY(run_slabs(c, nullptr, nullptr, true, mask01, true));                  // corr_0(d), corr_1(d) from the compact d
+        FixupParams f{};
+        f.x = x; f.u = c->u; f.cx0 = c->cx.buf[0]; f.cx1 = c->cx.buf[1]; f.e0 = e0; f.e1 = e1; f.alpha = (float)c->alpha;
+        f.partials = c->partials; f.slot0 = nb5; f.reduce_mode = RED_RESIDUAL; f.state = c->state; f.hist = c->hist_dev;
+        f.check_done = 1;
+        const double rows = (double)corr_elems(g, 0) + (double)corr_elems(g, 1);
+        KernelScope ks(c, "fixup_slab_rows", 40.0 * rows);
+        MBS_CUDA(c, launch_fixup(g, f, fixup_blocks(g, e0, e1, c->num_sms), c->stream));
+    }
+    return MBS_OK;
+}
+
+static int run_iteration(mbs_ctx* c, const cf* y, cf* x) {
+    return (c->fused && fused_available(c)) ? run_iteration_fused(c, y, x) : run_iteration_unfused(c, y, x);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -603,6 +682,10 @@ static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, do
     init.nu2 = nu > 0 ? nu * nu : 0.0; init.last_sum = 0;
     c->state_pinned[0] = init;
     MBS_CUDA(c, cudaMemcpyAsync(c->state, &c->state_pinned[0], sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
+    {
+        KernelScope ks(c, "source_row_mask", 8.0 * (double)c->g.voxels);
+        MBS_CUDA(c, launch_row_mask(y, c->ymask, c->g.voxels / c->g.N[2], c->g.N[2], c->stream));
+    }
     if (!(nu > 0)) {
         { KernelScope ks(c, "scale_copy", 16.0 * (double)c->g.voxels); MBS_CUDA(c, launch_scale_copy(y, c->u, to_cf(-c->c), c->g.voxels, c->stream)); }
         MBS_TRY(run_propagator(c, c->u, 1, false));
@@ -646,7 +729,7 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
         // enqueue one batch, then look at the poll of the PREVIOUS batch (one batch of lookahead keeps the GPU busy)
         const int batch = std::min(interval, max_iter - enqueued);
         if (batch > 0 && !final_done) {
-            for (int i = 0; i < batch; ++i) MBS_TRY(run_iteration_unfused(c, y, x));
+            for (int i = 0; i < batch; ++i) MBS_TRY(run_iteration(c, y, x));
             enqueued += batch;
             MBS_CUDA(c, cudaMemcpyAsync(&c->state_pinned[slot], c->state, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
             MBS_CUDA(c, cudaEventRecord(c->ev_poll[slot], c->stream));
@@ -701,7 +784,7 @@ extern "C" int mbs_iterate(mbs_ctx* c, const void* y_device, void* x_device, int
     MBS_TRY(ensure_history(c, n_iter));
     MBS_TRY(begin_solve(c, (const cf*)y_device, -1.0, n_iter, nu));
     MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
-    for (int i = 0; i < n_iter; ++i) MBS_TRY(run_iteration_unfused(c, (const cf*)y_device, (cf*)x_device));
+    for (int i = 0; i < n_iter; ++i) MBS_TRY(run_iteration(c, (const cf*)y_device, (cf*)x_device));
     MBS_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));
     DevState fin{};

@@ -2,6 +2,8 @@
 // size with -DMBS_FFT_SIZE=<M> (build.py) so the sizes build in parallel.
 #include "fft_plans.h"
 #include "mbs_internal.h"
+#include "fused_kernels.cuh"
+#include "fft_tma.cuh"
 
 #ifndef MBS_FFT_SIZE
 #error "compile with -DMBS_FFT_SIZE=<M>"
@@ -22,6 +24,24 @@ __global__ void __launch_bounds__(NT) k_fft_strided(cf* __restrict__ data, const
     fft_strided_body<PL, C, MODE>(data, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
 }
 
+// TMA-fed variant (fft_tma.cuh): persistent CTAs, NSTAGE shared-memory stages
+constexpr int tma_stages() {
+    const size_t stage = (size_t)PL::M * C * sizeof(cf);
+    const size_t budget = 220 * 1024;
+    return stage * 3 <= budget ? 3 : (stage * 2 <= budget ? 2 : 0);
+}
+constexpr int NSTAGE = tma_stages();
+
+template <int MODE>
+__global__ void __launch_bounds__(NT) k_fft_strided_tma(const __grid_constant__ CUtensorMap tmap, const StridedGeom g,
+                                                        const SymbolParams sp, const cf* __restrict__ tw,
+                                                        const int* __restrict__ done) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    if (done && *done) return;
+    if constexpr (NSTAGE >= 2)
+        fft_strided_tma_body<PL, C, MODE, (NSTAGE >= 2 ? NSTAGE : 2)>(&tmap, g, sp, tw, reinterpret_cast<cf*>(smem_raw));
+}
+
 template <int MODE>
 __global__ void __launch_bounds__(NT) k_fft_contig(const cf* src, cf* dst, const ContigGeom g,
                                                    const SymbolParams sp, const cf* __restrict__ tw,
@@ -31,22 +51,57 @@ __global__ void __launch_bounds__(NT) k_fft_contig(const cf* src, cf* dst, const
     fft_contig_body<PL, C, MODE>(src, dst, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
 }
 
+template <int MODE>
+__global__ void __launch_bounds__(NT) k_fused(const FusedParams p, const cf* __restrict__ tw, const int* __restrict__ done) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[32];
+    if (done && *done) return;
+    fused_contig_body<PL, C, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
+}
+
+// Opt in to the dynamic shared memory a kernel needs and query its occupancy; cached per (kernel, size).
+// (The attribute must be raised again when a later launch needs more than the size it was set to.)
 template <class K>
 cudaError_t prepare(K kernel, size_t smem, int* blocks_per_sm) {
-    static thread_local const void* done_for[16];
-    static thread_local int bps_for[16];
-    static thread_local int n_done = 0;
-    for (int i = 0; i < n_done; ++i)
-        if (done_for[i] == (const void*)kernel) { *blocks_per_sm = bps_for[i]; return cudaSuccess; }
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
+    struct Entry { const void* fn; size_t smem; size_t attr; int bps; };
+    static thread_local Entry cache[16];
+    static thread_local int n_cached = 0;
+    size_t attr = 0;
+    for (int i = 0; i < n_cached; ++i) {
+        if (cache[i].fn != (const void*)kernel) continue;
+        if (cache[i].smem == smem) { *blocks_per_sm = cache[i].bps; return cudaSuccess; }
+        if (cache[i].attr > attr) attr = cache[i].attr;
+    }
+    cudaError_t e;
+    if (smem > attr) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr = smem;
+    }
     int bps = 1;
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, NT, smem);
     if (e != cudaSuccess) return e;
     if (bps < 1) bps = 1;
-    if (n_done < 16) { done_for[n_done] = (const void*)kernel; bps_for[n_done] = bps; ++n_done; }
+    if (n_cached < 16) cache[n_cached++] = Entry{(const void*)kernel, smem, attr, bps};
     *blocks_per_sm = bps;
     return cudaSuccess;
+}
+
+template <int MODE>
+cudaError_t run_strided_tma(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, const int* done,
+                            int num_sms, cudaStream_t st) {
+    CUtensorMap map;
+    cudaError_t e = make_strided_tensor_map(&map, data, g, PL::M, C);
+    if (e != cudaSuccess) return e;
+    const size_t smem = tma_smem_bytes<PL, C, (NSTAGE >= 2 ? NSTAGE : 2)>();
+    int bps = 1;
+    e = prepare(k_fft_strided_tma<MODE>, smem, &bps);
+    if (e != cudaSuccess) return e;
+    long long nb = (long long)num_sms * bps;
+    if (nb > g.n_tiles) nb = g.n_tiles;
+    if (nb < 1) return cudaSuccess;
+    k_fft_strided_tma<MODE><<<(unsigned)nb, NT, smem, st>>>(map, g, sp, tw, done);
+    return cudaGetLastError();
 }
 
 template <int MODE>
@@ -77,8 +132,61 @@ cudaError_t run_contig(const cf* src, cf* dst, const ContigGeom& g, const Symbol
     return cudaGetLastError();
 }
 
+template <int MODE>
+cudaError_t fused_grid(int t, long long n_tiles, int num_sms, int* nb_out, size_t* smem_out) {
+    const size_t smem = sizeof(cf) * fused_smem_elems<PL, C>(t);
+    int bps = 1;
+    cudaError_t e = prepare(k_fused<MODE>, smem, &bps);
+    if (e != cudaSuccess) return e;
+    long long nb = (long long)num_sms * bps;
+    if (nb > n_tiles) nb = n_tiles;
+    if (nb > MBS_MAX_PARTIALS / 2) nb = MBS_MAX_PARTIALS / 2;
+    if (nb < 1) nb = 1;
+    *nb_out = (int)nb;
+    *smem_out = smem;
+    return cudaSuccess;
+}
+
+template <int MODE>
+cudaError_t run_fused(const FusedParams& p, const cf* tw, const int* done, int num_sms, cudaStream_t st) {
+    int nb = 1;
+    size_t smem = 0;
+    cudaError_t e = fused_grid<MODE>(p.t, p.n_tiles, num_sms, &nb, &smem);
+    if (e != cudaSuccess) return e;
+    k_fused<MODE><<<(unsigned)nb, NT, smem, st>>>(p, tw, done);
+    return cudaGetLastError();
+}
+
+cudaError_t fused_entry(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st) {
+    switch (mode) {
+        case FUSED_S1: return run_fused<FUSED_S1>(p, tw, done, num_sms, st);
+        case FUSED_S5: return run_fused<FUSED_S5>(p, tw, done, num_sms, st);
+        default: return run_fused<FUSED_1D>(p, tw, done, num_sms, st);
+    }
+}
+
+int fused_blocks_entry(int mode, int t, long long n_tiles, int num_sms) {
+    int nb = 1;
+    size_t smem = 0;
+    cudaError_t e;
+    switch (mode) {
+        case FUSED_S1: e = fused_grid<FUSED_S1>(t, n_tiles, num_sms, &nb, &smem); break;
+        case FUSED_S5: e = fused_grid<FUSED_S5>(t, n_tiles, num_sms, &nb, &smem); break;
+        default: e = fused_grid<FUSED_1D>(t, n_tiles, num_sms, &nb, &smem); break;
+    }
+    return e == cudaSuccess ? nb : -1;
+}
+
 cudaError_t strided_entry(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, int mode,
-                          const int* done, int num_sms, cudaStream_t st) {
+                          const int* done, int num_sms, int use_tma, cudaStream_t st) {
+    // TMA needs 16-byte multiples for the global strides (inner even) and a 16-byte aligned base
+    if (use_tma && NSTAGE >= 2 && g.inner % 2 == 0 && (reinterpret_cast<uintptr_t>(data) & 15) == 0) {
+        switch (mode) {
+            case FFT_FWD: return run_strided_tma<FFT_FWD>(data, g, sp, tw, done, num_sms, st);
+            case FFT_INV: return run_strided_tma<FFT_INV>(data, g, sp, tw, done, num_sms, st);
+            default: return run_strided_tma<FFT_MID>(data, g, sp, tw, done, num_sms, st);
+        }
+    }
     switch (mode) {
         case FFT_FWD: return run_strided<FFT_FWD>(data, g, sp, tw, done, num_sms, st);
         case FFT_INV: return run_strided<FFT_INV>(data, g, sp, tw, done, num_sms, st);
@@ -99,6 +207,7 @@ cudaError_t contig_entry(const cf* src, cf* dst, const ContigGeom& g, const Symb
 
 #define MBS_CAT2(a, b) a##b
 #define MBS_CAT(a, b) MBS_CAT2(a, b)
-extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {MBS_FFT_SIZE, C, strided_entry, contig_entry};
+extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {MBS_FFT_SIZE, C, strided_entry, contig_entry, fused_entry,
+                                                                    fused_blocks_entry};
 
 }  // namespace mbs

@@ -10,63 +10,9 @@
 #include <math_constants.h>
 
 #include "mbs_internal.h"
+#include "reduce.cuh"
 
 namespace mbs {
-
-// ---------------------------------------------------------------------------------------------
-// block reduction helpers (fixed order -> bitwise reproducible sums)
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
-
-__device__ __forceinline__ double block_sum(double v, double* red /*[32]*/) {
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    v = warp_sum(v);
-    __syncthreads();
-    if (lane == 0) red[wid] = v;
-    __syncthreads();
-    const int nw = (blockDim.x + 31) >> 5;
-    double r = (threadIdx.x < nw) ? red[threadIdx.x] : 0.0;
-    if (wid == 0) r = warp_sum(r);
-    return r;  // valid in warp 0
-}
-
-// Called by every block with its partial sum; the last block to arrive adds all partials in index
-// order and finishes the reduction (no extra launch, no host round trip).
-__device__ void finish_reduction(double block_partial, const PointwiseParams& p, double* red) {
-    __shared__ int s_last;
-    if (threadIdx.x == 0) {
-        p.partials[blockIdx.x] = block_partial;
-        __threadfence();
-        const unsigned int ticket = atomicAdd(&p.state->ticket, 1u);
-        s_last = (ticket == gridDim.x - 1);
-    }
-    __syncthreads();
-    if (!s_last) return;
-    __threadfence();
-    double acc = 0.0;
-    for (int i = threadIdx.x; i < (int)gridDim.x; i += blockDim.x) acc += __ldcg(&p.partials[i]);
-    const double total = block_sum(acc, red);
-    if (threadIdx.x == 0) {
-        DevState* s = p.state;
-        s->ticket = 0;
-        s->last_sum = total;
-        if (p.reduce == RED_NU2) {
-            s->nu2 = total;
-        } else if (p.reduce == RED_RESIDUAL) {
-            const double eps = sqrt(total / s->nu2);
-            const int n = s->iter;
-            if (p.hist) p.hist[n] = eps;
-            s->iter = n + 1;
-            if (!(eps == eps) || eps > 1.0e300) s->done = 3;      // NaN / Inf
-            else if (eps < s->tol) s->done = 1;
-            else if (n + 1 >= s->max_iter) s->done = 2;
-        }
-    }
-}
 
 // ---------------------------------------------------------------------------------------------
 // pointwise pass
@@ -195,7 +141,7 @@ __global__ void __launch_bounds__(PW_THREADS) k_pointwise(const GridDesc g, cons
     }
     if (p.reduce) {
         const double bs = block_sum((double)acc, red);
-        finish_reduction(bs, p, red);
+        grid_reduce_finish(bs, p.partials, 0, (int)gridDim.x, 1, p.reduce, p.state, p.hist, red);
     }
 }
 
@@ -249,11 +195,17 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab(const GridDesc g, const S
             if (g.per[ax]) nb = (nb + S) % S;
             else has_nb = false;
         }
-        const long long base_o = o * (long long)g.N[ax] * inner + in_i;
         // side 1 reads the FIRST t points of own and neighbour; side 0 reads the LAST t points
-        const long long off = side ? 0 : (long long)(M - t);
-        const long long own0 = base_o + ((long long)s * M + off) * axis_stride;
-        const long long nb0 = base_o + ((long long)nb * M + off) * axis_stride;
+        long long own0, nb0;
+        if (p.compact_in) {   // input already in the compact [outer][S*2t][inner] layout
+            own0 = ((o * S + s) * 2 * t + (side ? 0 : t)) * inner + in_i;
+            nb0 = ((o * S + nb) * 2 * t + (side ? 0 : t)) * inner + in_i;
+        } else {
+            const long long base_o = o * (long long)g.N[ax] * inner + in_i;
+            const long long off = side ? 0 : (long long)(M - t);
+            own0 = base_o + ((long long)s * M + off) * axis_stride;
+            nb0 = base_o + ((long long)nb * M + off) * axis_stride;
+        }
         cf dv[TT];
 #pragma unroll
         for (int q = 0; q < TT; ++q) {
@@ -305,10 +257,16 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_generic(const GridDesc g,
             if (g.per[ax]) nb = (nb + S) % S;
             else has_nb = false;
         }
-        const long long base_o = o * (long long)g.N[ax] * inner + in_i;
-        const long long off = side ? 0 : (long long)(M - t);
-        const long long own0 = base_o + ((long long)s * M + off) * inner;
-        const long long nb0 = base_o + ((long long)nb * M + off) * inner;
+        long long own0, nb0;
+        if (p.compact_in) {
+            own0 = ((o * S + s) * 2 * t + (side ? 0 : t)) * inner + in_i;
+            nb0 = ((o * S + nb) * 2 * t + (side ? 0 : t)) * inner + in_i;
+        } else {
+            const long long base_o = o * (long long)g.N[ax] * inner + in_i;
+            const long long off = side ? 0 : (long long)(M - t);
+            own0 = base_o + ((long long)s * M + off) * inner;
+            nb0 = base_o + ((long long)nb * M + off) * inner;
+        }
         float sr = 0.f, si = 0.f;
         for (int q = 0; q < t; ++q) {
             cf own = p.in[own0 + q * inner];
@@ -346,6 +304,128 @@ cudaError_t launch_slab(const GridDesc& g, const SlabParams& p, cudaStream_t st)
             k_slab_generic<<<(unsigned)nb2, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items);
         }
     }
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// fix-up of the fused last sweep: on every row that lies in a slab of axis 0 or 1,
+//   r = r_part - corr_0(d) - corr_1(d),  |r|^2 partial sums,  x <- x - alpha r      (a7-a9)
+// r_part = B_diag d - corr_2(d) was left in u by the fused sweep; corr_0(d), corr_1(d) are in the compact
+// buffers.  Rows are enumerated without a list: set A = {i0 edge of axis 0} x all i1, then
+// set B = {i0 not an edge of axis 0} x {i1 edge of axis 1}.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int edge_index(int q, int M, int t) {   // q in [0, S*2t) -> grid index
+    const int s = q / (2 * t), e = q - s * 2 * t;
+    return s * M + (e < t ? e : M - 2 * t + e);
+}
+
+template <int VEC>
+__global__ void __launch_bounds__(PW_THREADS) k_fixup(const GridDesc g, const FixupParams p) {
+    __shared__ double red[32];
+    if (p.check_done && p.state->done) return;
+    const int t = g.t;
+    const int nE0 = p.e0 ? g.S[0] * 2 * t : 0, nE1 = p.e1 ? g.S[1] * 2 * t : 0;
+    const long long rowsA = (long long)nE0 * g.N[1];
+    const long long rowsB = (long long)(g.N[0] - nE0) * nE1;
+    const int chunk_len = PW_THREADS * VEC;
+    const int nchunks = (g.N[2] + chunk_len - 1) / chunk_len;
+    const long long n_work = (rowsA + rowsB) * nchunks;
+    float acc = 0.f;
+    for (long long work = blockIdx.x; work < n_work; work += gridDim.x) {
+        const int chunk = (int)(work % nchunks);
+        const long long rid = work / nchunks;
+        int i0, i1, q0 = -1, q1 = -1;
+        if (rid < rowsA) {
+            q0 = (int)(rid / g.N[1]);
+            i1 = (int)(rid - (long long)q0 * g.N[1]);
+            i0 = edge_index(q0, g.M[0], t);
+            if (p.e1) q1 = edge_slot(i1, g.M[1], t);
+        } else {
+            const long long rb = rid - rowsA;
+            const int k0 = (int)(rb / nE1);          // k0-th non-edge index of axis 0
+            q1 = (int)(rb - (long long)k0 * nE1);
+            i1 = edge_index(q1, g.M[1], t);
+            if (p.e0) {
+                const int w = g.M[0] - 2 * t;
+                const int s = k0 / w;
+                i0 = s * g.M[0] + t + (k0 - s * w);
+            } else {
+                i0 = k0;
+            }
+        }
+        const int i2 = chunk * chunk_len + threadIdx.x * VEC;
+        if (i2 >= g.N[2]) continue;
+        const long long idx = ((long long)i0 * g.N[1] + i1) * g.N[2] + i2;
+        cf r[VEC], xv[VEC];
+        load_vec<VEC>(p.u + idx, r);
+        load_vec<VEC>(p.x + idx, xv);
+        if (q0 >= 0) {
+            cf cc[VEC];
+            load_vec<VEC>(p.cx0 + ((long long)q0 * g.N[1] + i1) * g.N[2] + i2, cc);
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) r[v] = csub(r[v], cc[v]);
+        }
+        if (q1 >= 0) {
+            cf cc[VEC];
+            load_vec<VEC>(p.cx1 + ((long long)i0 * nE1 + q1) * g.N[2] + i2, cc);
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) r[v] = csub(r[v], cc[v]);
+        }
+#pragma unroll
+        for (int v = 0; v < VEC; ++v) {
+            acc += r[v].x * r[v].x + r[v].y * r[v].y;
+            xv[v] = make_float2(xv[v].x - p.alpha * r[v].x, xv[v].y - p.alpha * r[v].y);
+        }
+        store_vec<VEC>(p.x + idx, xv);
+    }
+    const double bs = block_sum((double)acc, red);
+    grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, 1, p.reduce_mode, p.state, p.hist, red);
+}
+
+int fixup_blocks(const GridDesc& g, int e0, int e1, int num_sms) {
+    const int vec = (g.N[2] % 2 == 0) ? 2 : 1;
+    const int chunk_len = PW_THREADS * vec;
+    const long long nchunks = (g.N[2] + chunk_len - 1) / chunk_len;
+    const long long nE0 = e0 ? g.S[0] * 2 * g.t : 0, nE1 = e1 ? g.S[1] * 2 * g.t : 0;
+    const long long n_work = (nE0 * g.N[1] + (g.N[0] - nE0) * nE1) * nchunks;
+    long long nb = (long long)num_sms * 8;
+    if (nb > MBS_MAX_PARTIALS / 2) nb = MBS_MAX_PARTIALS / 2;
+    if (nb > n_work) nb = n_work;
+    return (int)(nb < 1 ? 1 : nb);
+}
+
+cudaError_t launch_fixup(const GridDesc& g, const FixupParams& p, int nblocks, cudaStream_t st) {
+    if (g.N[2] % 2 == 0) k_fixup<2><<<nblocks, PW_THREADS, 0, st>>>(g, p);
+    else k_fixup<1><<<nblocks, PW_THREADS, 0, st>>>(g, p);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// mask[row] = 1 if the row of y (N2 contiguous voxels) holds a non-zero value.  Point, line and plane
+// sources leave almost every row empty; the fused first sweep skips the load of y there.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_row_mask(const cf* __restrict__ y, unsigned char* __restrict__ mask,
+                                                  const long long rows, const int N2) {
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long row = warp0; row < rows; row += nwarps) {
+        const cf* yr = y + row * N2;
+        bool nz = false;
+        for (int i = lane; i < N2; i += 32) {
+            const cf v = yr[i];
+            nz = nz || (v.x != 0.f) || (v.y != 0.f);
+        }
+        nz = __any_sync(0xffffffffu, nz);
+        if (lane == 0) mask[row] = nz ? 1 : 0;
+    }
+}
+
+cudaError_t launch_row_mask(const cf* y, unsigned char* mask, long long rows, int N2, cudaStream_t st) {
+    long long nb = (rows + 7) / 8;
+    if (nb > 148 * 16) nb = 148 * 16;
+    if (nb < 1) nb = 1;
+    k_row_mask<<<(unsigned)nb, 256, 0, st>>>(y, mask, rows, N2);
     return cudaGetLastError();
 }
 

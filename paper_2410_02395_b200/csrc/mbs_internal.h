@@ -1,5 +1,6 @@
 // mbs_internal.h -- shared declarations of the library's translation units (not installed).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -75,13 +76,33 @@ struct SlabParams {
     const float* Kh;   // t x t, K_t / h^2, row-major (row a = last-edge index, column b = first-edge index)
     cf c;              // scale factor c of Eq. (9)
     int axis;
+    int compact_in;    // 1: `in` is already a compact [outer][S*2t][inner] buffer (fix-up of the fused sweep)
     const DevState* state;
+    int check_done;
+};
+
+// fix-up of the fused last sweep on the slab rows of axes 0 and 1 (kernels.cu: k_fixup)
+struct FixupParams {
+    cf* x;
+    const cf* u;       // r_part on the slab rows
+    const cf* cx0;     // corr_0(d), corr_1(d), compact
+    const cf* cx1;
+    int e0, e1;
+    float alpha;
+    double* partials;
+    int slot0;         // first partial slot of this launch; slots below hold the fused sweep's partials
+    int reduce_mode;
+    DevState* state;
+    double* hist;
     int check_done;
 };
 
 // launchers implemented in kernels.cu
 cudaError_t launch_pointwise(const GridDesc& g, const PointwiseParams& p, int num_sms, cudaStream_t st);
 cudaError_t launch_slab(const GridDesc& g, const SlabParams& p, cudaStream_t st);
+int fixup_blocks(const GridDesc& g, int e0, int e1, int num_sms);
+cudaError_t launch_fixup(const GridDesc& g, const FixupParams& p, int nblocks, cudaStream_t st);
+cudaError_t launch_row_mask(const cf* y, unsigned char* mask, long long rows, int N2, cudaStream_t st);
 cudaError_t launch_scale_copy(const cf* in, cf* out, cf scale, long long n, cudaStream_t st);
 
 struct SetupParams {
@@ -98,15 +119,54 @@ struct SetupParams {
 cudaError_t launch_setup(const GridDesc& g, const SetupParams& p, int pass, double* out, cf* bdiag, int nblocks,
                          cudaStream_t st);
 
+// fused first / last sweep along the contiguous axis (fused_kernels.cuh)
+enum FusedMode { FUSED_S1 = 0, FUSED_S5 = 1, FUSED_1D = 2 };
+
+struct FusedParams {
+    cf* x;               // iterate: read by S1; read and updated in place by S5 / 1D
+    const cf* bdiag;     // B_diag = 1 - c (k^2 - k0^2)
+    const cf* y;         // physical source (S1 / 1D) or nullptr
+    const unsigned char* ymask;   // per grid row: 0 = the row of y is all zero (skip its load); nullptr = unknown
+    cf ysc;              // y_vec = ysc * y = -c y
+    cf* u;               // S1: output; S5: input u' lines, output r_part on slab rows
+    int N1, N2;          // extents of axes 1 and 2 (N2 = S2 * M)
+    int S2, a2, per2;    // subdomains, a_d and periodic flag of the last axis
+    int t;               // correction points
+    int e0, e1;          // 1 if axis 0 / 1 has edge corrections
+    int M0, M1, S1;
+    const cf* cx0;       // S1: corr_0(x), compact [S0*2t][N1][N2]
+    const cf* cx1;       // S1: corr_1(x), compact [N0][S1*2t][N2]
+    cf* ds0;             // S5: d at the axis-0 slab rows, same layouts
+    cf* ds1;
+    const float* Kh;     // K_t / h^2, t x t row-major
+    cf c;                // scale factor of Eq. (9)
+    float alpha;
+    SymbolParams sp;     // 1D: Fourier kernel
+    long long n_lines;   // voxels / M
+    long long n_tiles;
+    // reduction
+    double* partials;
+    int slot0, n_total, finish, reduce_mode;
+    DevState* state;
+    double* hist;
+};
+
 // FFT registry (fft_inst.cu compiled once per size, fft_registry.cu)
 struct FftEntry {
     int M;
     int C;   // lines per tile
     cudaError_t (*strided)(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, int mode,
-                           const int* done, int num_sms, cudaStream_t st);
+                           const int* done, int num_sms, int use_tma, cudaStream_t st);
     cudaError_t (*contig)(const cf* src, cf* dst, const ContigGeom& g, const SymbolParams& sp, const cf* tw, int mode,
                           const int* done, int num_sms, cudaStream_t st);
+    // fused sweep (FusedMode); *blocks_out = grid size used (number of residual partials written)
+    cudaError_t (*fused)(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st);
+    int (*fused_blocks)(int mode, int t, long long n_tiles, int num_sms);
 };
 const FftEntry* fft_lookup(int M);
+
+// Tensor map of `data` viewed as [n_outer][n_seg*M][inner] for the TMA-fed strided sweep (fft_registry.cu):
+// float32 dims {2*inner, n_seg*M, n_outer}, box {2*C, M / ceil(M/256), 1}.
+cudaError_t make_strided_tensor_map(CUtensorMap* out, const cf* data, const StridedGeom& g, int M, int C);
 
 }  // namespace mbs

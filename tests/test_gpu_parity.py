@@ -87,6 +87,39 @@ def test_operator_parity(B, orc, shape, S, W, t, periodic):
     s.close()
 
 
+ITERATION_CASES = OPERATOR_CASES + [
+    ((512,), (4,), (8,), 8, None),
+    ((8, 8, 256), (1, 1, 2), (0, 0, 8), 8, (1, 1, 0)),       # periodic single-domain axes 0, 1: no slab rows
+    ((48, 40, 64), (3, 1, 2), (4, 4, 4), 8, None),            # ragged tile tail: 48*40*2 lines is not a multiple of 16
+    ((32, 32, 320), (2, 2, 1), (4, 4, 8), 8, None),
+]
+
+
+@pytest.mark.parametrize("fused,tma", [(1, 1), (0, 1), (1, 0)])
+@pytest.mark.parametrize("shape,S,W,t,periodic", ITERATION_CASES)
+def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma):
+    """A few updates of Eq. (6) from a random start with a dense random source, fused sweeps and
+    one-kernel-per-step path, against the oracle's iterates: every step of SURVEY 8(a) on every geometry."""
+    import torch
+    s, o, n = make_pair(B, orc, shape, S, W, t, periodic, seed=11)
+    s.set_option(B.MBS_OPT_FUSED, fused)
+    s.set_option(B.MBS_OPT_TMA, tma)
+    y = workloads.random_field(shape, 21)
+    x0 = workloads.random_field(shape, 22)
+    n_it = 6
+    x_ref, h_ref = o.solve(y, x0=x0, tol=0.0, max_iter=n_it)
+    yd = torch.from_numpy(y).cuda()
+    xd = torch.from_numpy(x0).cuda()
+    hist = s.iterate(yd, xd, n_it)
+    assert np.allclose(hist, h_ref, rtol=2e-5), (hist, h_ref)
+    assert rel(xd.cpu().numpy(), x_ref) <= OP_TOL, rel(xd.cpu().numpy(), x_ref)
+    # the same through mbs_solve (stop flag path): identical history, bit for bit
+    x2, hist2, rc = s.solve(y, x0=x0, tol=0.0, max_iter=n_it)
+    assert rc == B.MBS_ERR_NOT_CONVERGED
+    assert np.array_equal(hist2, hist) and torch.equal(x2, xd)
+    s.close()
+
+
 def test_B_is_diagonal_plus_slabs_only(B, orc):
     """V touches only the diagonal and the 2t edge points of each subdomain: away from the
     edges B u = B_diag u exactly as the oracle computes it; at the edges the slab terms are non-zero."""
@@ -130,13 +163,20 @@ def count_slack(h_ref, thr, floor):
     return 1 + int(np.ceil(1.5 * (floor / thr) ** 2 / (2.0 * rate)))
 
 
+_ORACLE_CACHE = {}
+
+
+@pytest.mark.parametrize("fused", [1, 0])
 @pytest.mark.parametrize("name,make", SOLVE_CASES)
-def test_solve_parity(B, orc, name, make):
+def test_solve_parity(B, orc, name, make, fused):
     w = make()
     n, y = w.make_medium(), w.make_source()
     o = orc.from_workload(w, n)
-    x_ref, h_ref = o.solve(y, tol=w.tol, max_iter=w.max_iter)
+    if name not in _ORACLE_CACHE:
+        _ORACLE_CACHE[name] = o.solve(y, tol=w.tol, max_iter=w.max_iter)
+    x_ref, h_ref = _ORACLE_CACHE[name]
     s = B.Solver.from_workload(w)
+    s.set_option(B.MBS_OPT_FUSED, fused)
     s.set_potential(n)
     # (1) the complex64 floor of this case: run past the oracle's stop without a stop test
     _, h_long, rc = s.solve(y, tol=0.0, max_iter=len(h_ref) + 300)
