@@ -47,6 +47,7 @@ def parse_args():
     ap.add_argument("--warmup", type=int, default=None)
     ap.add_argument("--config", type=int, default=5, choices=(3, 4, 5))
     ap.add_argument("--impl", default="b200", choices=("b200", "reference"))
+    ap.add_argument("--shape", default=None, help="override the grid, e.g. 256,512,1024 (profiling runs; not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-converge", action="store_true")
@@ -187,7 +188,7 @@ def run_b200(args):
     W = args.warmup if args.warmup is not None else 3
     W = max(W, 3)
 
-    w = workloads.config(args.config)
+    w = workloads.config(args.config, shape=tuple(int(v) for v in args.shape.split(",")) if args.shape else None)
     t0 = time.perf_counter()
     n_map, y = w.make_medium(), w.make_source()
     t_gen = time.perf_counter() - t0

@@ -15,7 +15,8 @@ from typing import Optional, Sequence, Tuple
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libmbs_b200.so")
+# MBS_B200_LIB lets a developer load another build of the same library (kernel tuning); default: in-tree
+LIB_PATH = os.environ.get("MBS_B200_LIB") or os.path.join(_HERE, "libmbs_b200.so")
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(

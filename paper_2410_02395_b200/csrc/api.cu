@@ -506,7 +506,7 @@ static int run_fft_contig(mbs_ctx* c, cf* buf, int mode, int inverse, bool in_lo
     ContigGeom cg{};
     const FftEntry* e = c->fft[2];
     cg.n_lines = g.voxels / g.M[2];
-    cg.n_tiles = (cg.n_lines + e->C - 1) / e->C;
+    cg.n_tiles = (cg.n_lines + e->CC - 1) / e->CC;
     SymbolParams s2 = make_symbol(c, inverse);
     s2.tab_axis = c->p2_dev[2];
     static const char* names[3] = {"fft_contig_fwd", "fft_contig_inv", "fft_contig_mid"};
@@ -524,7 +524,7 @@ static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, b
     for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
     for (int d = 0; d < ax; ++d) outer *= g.N[d];
     sg.stride = inner; sg.outer_stride = (long long)g.N[ax] * inner; sg.n_outer = (int)outer; sg.n_seg = g.S[ax];
-    sg.inner = (int)inner; sg.tiles_inner = (int)((inner + e->C - 1) / e->C);
+    sg.inner = (int)inner; sg.tiles_inner = (int)((inner + e->CS - 1) / e->CS);
     sg.n_tiles = outer * g.S[ax] * sg.tiles_inner;
     SymbolParams s2 = make_symbol(c, inverse);
     s2.tab_axis = c->p2_dev[ax];
@@ -584,7 +584,7 @@ static int run_iteration_unfused(mbs_ctx* c, const cf* y, cf* x) {
 }
 
 // The fused path needs whole grid rows inside one tile of the contiguous-axis kernel.
-static bool fused_available(const mbs_ctx* c) { return c->fft[2]->C % c->g.S[2] == 0; }
+static bool fused_available(const mbs_ctx* c) { return c->fft[2]->CC % c->g.S[2] == 0; }
 
 // one iteration of Eq. (6), fused sweeps (112 B/voxel ledger of DESIGN.md section 5)
 static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
@@ -600,7 +600,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     p.Kh = c->Kh_dev; p.c = to_cf(c->c); p.alpha = (float)c->alpha;
     p.sp = make_symbol(c, 1); p.sp.tab_axis = c->p2_dev[2];
     p.n_lines = g.voxels / g.M[2];
-    p.n_tiles = (p.n_lines + e->C - 1) / e->C;
+    p.n_tiles = (p.n_lines + e->CC - 1) / e->CC;
     p.partials = c->partials; p.state = c->state; p.hist = c->hist_dev; p.reduce_mode = RED_RESIDUAL;
     const double vb = 8.0 * (double)g.voxels;
     if (c->ndim == 1) {

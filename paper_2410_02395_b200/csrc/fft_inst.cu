@@ -13,56 +13,67 @@ namespace mbs {
 namespace {
 
 using PL = FftPlan<MBS_FFT_SIZE>::type;
-constexpr int C = FftPlan<MBS_FFT_SIZE>::C;
-constexpr int NT = PL::T * C;
+// tile widths: CS voxels per tile row of the strided sweeps, CC lines per tile of the contiguous sweeps
+#ifdef MBS_CS
+constexpr int CS = MBS_CS;
+#else
+constexpr int CS = FftPlan<MBS_FFT_SIZE>::CS;
+#endif
+#ifdef MBS_CC
+constexpr int CC = MBS_CC;
+#else
+constexpr int CC = FftPlan<MBS_FFT_SIZE>::CC;
+#endif
+constexpr int NTS = PL::T * CS;
+constexpr int NTC = PL::T * CC;
 
 template <int MODE>
-__global__ void __launch_bounds__(NT) k_fft_strided(cf* __restrict__ data, const StridedGeom g, const SymbolParams sp,
+__global__ void __launch_bounds__(NTS) k_fft_strided(cf* __restrict__ data, const StridedGeom g, const SymbolParams sp,
                                                     const cf* __restrict__ tw, const int* __restrict__ done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *done) return;
-    fft_strided_body<PL, C, MODE>(data, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
+    fft_strided_body<PL, CS, MODE>(data, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
 }
 
 // TMA-fed variant (fft_tma.cuh): persistent CTAs, NSTAGE shared-memory stages
 constexpr int tma_stages() {
-    const size_t stage = (size_t)PL::M * C * sizeof(cf);
+    const size_t stage = (size_t)PL::M * CS * sizeof(cf);
     const size_t budget = 220 * 1024;
     return stage * 3 <= budget ? 3 : (stage * 2 <= budget ? 2 : 0);
 }
 constexpr int NSTAGE = tma_stages();
 
 template <int MODE>
-__global__ void __launch_bounds__(NT) k_fft_strided_tma(const __grid_constant__ CUtensorMap tmap, const StridedGeom g,
+__global__ void __launch_bounds__(NTS) k_fft_strided_tma(const __grid_constant__ CUtensorMap tmap, const StridedGeom g,
                                                         const SymbolParams sp, const cf* __restrict__ tw,
                                                         const int* __restrict__ done) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     if (done && *done) return;
     if constexpr (NSTAGE >= 2)
-        fft_strided_tma_body<PL, C, MODE, (NSTAGE >= 2 ? NSTAGE : 2)>(&tmap, g, sp, tw, reinterpret_cast<cf*>(smem_raw));
+        fft_strided_tma_body<PL, CS, MODE, (NSTAGE >= 2 ? NSTAGE : 2)>(&tmap, g, sp, tw, reinterpret_cast<cf*>(smem_raw));
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(NT) k_fft_contig(const cf* src, cf* dst, const ContigGeom g,
+__global__ void __launch_bounds__(NTC) k_fft_contig(const cf* src, cf* dst, const ContigGeom g,
                                                    const SymbolParams sp, const cf* __restrict__ tw,
                                                    const int* __restrict__ done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *done) return;
-    fft_contig_body<PL, C, MODE>(src, dst, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
+    fft_contig_body<PL, CC, MODE>(src, dst, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
 }
 
 template <int MODE>
-__global__ void __launch_bounds__(NT) k_fused(const FusedParams p, const cf* __restrict__ tw, const int* __restrict__ done) {
+__global__ void __launch_bounds__(NTC) k_fused(const FusedParams p, const cf* __restrict__ tw, const int* __restrict__ done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     if (done && *done) return;
-    fused_contig_body<PL, C, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
+    fused_contig_body<PL, CC, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
 }
 
 // Opt in to the dynamic shared memory a kernel needs and query its occupancy; cached per (kernel, size).
 // (The attribute must be raised again when a later launch needs more than the size it was set to.)
 template <class K>
-cudaError_t prepare(K kernel, size_t smem, int* blocks_per_sm) {
+cudaError_t prepare(K kernel, int nthreads, size_t smem, int* blocks_per_sm) {
     struct Entry { const void* fn; size_t smem; size_t attr; int bps; };
     static thread_local Entry cache[16];
     static thread_local int n_cached = 0;
@@ -79,7 +90,7 @@ cudaError_t prepare(K kernel, size_t smem, int* blocks_per_sm) {
         attr = smem;
     }
     int bps = 1;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, NT, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, nthreads, smem);
     if (e != cudaSuccess) return e;
     if (bps < 1) bps = 1;
     if (n_cached < 16) cache[n_cached++] = Entry{(const void*)kernel, smem, attr, bps};
@@ -91,52 +102,52 @@ template <int MODE>
 cudaError_t run_strided_tma(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, const int* done,
                             int num_sms, cudaStream_t st) {
     CUtensorMap map;
-    cudaError_t e = make_strided_tensor_map(&map, data, g, PL::M, C);
+    cudaError_t e = make_strided_tensor_map(&map, data, g, PL::M, CS);
     if (e != cudaSuccess) return e;
-    const size_t smem = tma_smem_bytes<PL, C, (NSTAGE >= 2 ? NSTAGE : 2)>();
+    const size_t smem = tma_smem_bytes<PL, CS, (NSTAGE >= 2 ? NSTAGE : 2)>();
     int bps = 1;
-    e = prepare(k_fft_strided_tma<MODE>, smem, &bps);
+    e = prepare(k_fft_strided_tma<MODE>, NTS, smem, &bps);
     if (e != cudaSuccess) return e;
     long long nb = (long long)num_sms * bps;
     if (nb > g.n_tiles) nb = g.n_tiles;
     if (nb < 1) return cudaSuccess;
-    k_fft_strided_tma<MODE><<<(unsigned)nb, NT, smem, st>>>(map, g, sp, tw, done);
+    k_fft_strided_tma<MODE><<<(unsigned)nb, NTS, smem, st>>>(map, g, sp, tw, done);
     return cudaGetLastError();
 }
 
 template <int MODE>
 cudaError_t run_strided(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, const int* done,
                         int num_sms, cudaStream_t st) {
-    const size_t smem = sizeof(cf) * strided_smem_elems<PL, C>();
+    const size_t smem = sizeof(cf) * strided_smem_elems<PL, CS>();
     int bps = 1;
-    cudaError_t e = prepare(k_fft_strided<MODE>, smem, &bps);
+    cudaError_t e = prepare(k_fft_strided<MODE>, NTS, smem, &bps);
     if (e != cudaSuccess) return e;
     long long nb = (long long)num_sms * bps;
     if (nb > g.n_tiles) nb = g.n_tiles;
     if (nb < 1) return cudaSuccess;
-    k_fft_strided<MODE><<<(unsigned)nb, NT, smem, st>>>(data, g, sp, tw, done);
+    k_fft_strided<MODE><<<(unsigned)nb, NTS, smem, st>>>(data, g, sp, tw, done);
     return cudaGetLastError();
 }
 
 template <int MODE>
 cudaError_t run_contig(const cf* src, cf* dst, const ContigGeom& g, const SymbolParams& sp, const cf* tw,
                        const int* done, int num_sms, cudaStream_t st) {
-    const size_t smem = sizeof(cf) * contig_smem_elems<PL, C>();
+    const size_t smem = sizeof(cf) * contig_smem_elems<PL, CC>();
     int bps = 1;
-    cudaError_t e = prepare(k_fft_contig<MODE>, smem, &bps);
+    cudaError_t e = prepare(k_fft_contig<MODE>, NTC, smem, &bps);
     if (e != cudaSuccess) return e;
     long long nb = (long long)num_sms * bps;
     if (nb > g.n_tiles) nb = g.n_tiles;
     if (nb < 1) return cudaSuccess;
-    k_fft_contig<MODE><<<(unsigned)nb, NT, smem, st>>>(src, dst, g, sp, tw, done);
+    k_fft_contig<MODE><<<(unsigned)nb, NTC, smem, st>>>(src, dst, g, sp, tw, done);
     return cudaGetLastError();
 }
 
 template <int MODE>
 cudaError_t fused_grid(int t, long long n_tiles, int num_sms, int* nb_out, size_t* smem_out) {
-    const size_t smem = sizeof(cf) * fused_smem_elems<PL, C>(t);
+    const size_t smem = sizeof(cf) * fused_smem_elems<PL, CC>(t);
     int bps = 1;
-    cudaError_t e = prepare(k_fused<MODE>, smem, &bps);
+    cudaError_t e = prepare(k_fused<MODE>, NTC, smem, &bps);
     if (e != cudaSuccess) return e;
     long long nb = (long long)num_sms * bps;
     if (nb > n_tiles) nb = n_tiles;
@@ -153,7 +164,7 @@ cudaError_t run_fused(const FusedParams& p, const cf* tw, const int* done, int n
     size_t smem = 0;
     cudaError_t e = fused_grid<MODE>(p.t, p.n_tiles, num_sms, &nb, &smem);
     if (e != cudaSuccess) return e;
-    k_fused<MODE><<<(unsigned)nb, NT, smem, st>>>(p, tw, done);
+    k_fused<MODE><<<(unsigned)nb, NTC, smem, st>>>(p, tw, done);
     return cudaGetLastError();
 }
 
@@ -207,7 +218,7 @@ cudaError_t contig_entry(const cf* src, cf* dst, const ContigGeom& g, const Symb
 
 #define MBS_CAT2(a, b) a##b
 #define MBS_CAT(a, b) MBS_CAT2(a, b)
-extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {MBS_FFT_SIZE, C, strided_entry, contig_entry, fused_entry,
+extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {MBS_FFT_SIZE, CS, CC, strided_entry, contig_entry, fused_entry,
                                                                     fused_blocks_entry};
 
 }  // namespace mbs

@@ -8,19 +8,19 @@ namespace mbs {
 
 template <int M> struct FftPlan;
 //                                          M     P   radices...
-template <> struct FftPlan<8>    { using type = Plan<8,    8,  8>;            static constexpr int C = 64; };
-template <> struct FftPlan<16>   { using type = Plan<16,   8,  8, 2>;         static constexpr int C = 64; };
-template <> struct FftPlan<32>   { using type = Plan<32,   8,  8, 4>;         static constexpr int C = 32; };
-template <> struct FftPlan<64>   { using type = Plan<64,   8,  8, 8>;         static constexpr int C = 16; };
-template <> struct FftPlan<128>  { using type = Plan<128,  16, 16, 8>;        static constexpr int C = 16; };
-template <> struct FftPlan<256>  { using type = Plan<256,  16, 16, 16>;       static constexpr int C = 16; };
-template <> struct FftPlan<512>  { using type = Plan<512,  16, 16, 16, 2>;    static constexpr int C = 16; };
-template <> struct FftPlan<1024> { using type = Plan<1024, 16, 16, 16, 4>;    static constexpr int C = 8;  };
-template <> struct FftPlan<40>   { using type = Plan<40,   20, 20, 2>;        static constexpr int C = 64; };
-template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        static constexpr int C = 32; };
-template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int C = 16; };
-template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int C = 16; };
-template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int C = 16; };
+template <> struct FftPlan<8>    { using type = Plan<8,    8,  8>;            static constexpr int CS = 64, CC = 64; };
+template <> struct FftPlan<16>   { using type = Plan<16,   8,  8, 2>;         static constexpr int CS = 64, CC = 64; };
+template <> struct FftPlan<32>   { using type = Plan<32,   8,  8, 4>;         static constexpr int CS = 32, CC = 32; };
+template <> struct FftPlan<64>   { using type = Plan<64,   8,  8, 8>;         static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<128>  { using type = Plan<128,  16, 16, 8>;        static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<256>  { using type = Plan<256,  16, 16, 16>;       static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<512>  { using type = Plan<512,  16, 16, 16, 2>;    static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<1024> { using type = Plan<1024, 16, 16, 16, 4>;    static constexpr int CS = 8, CC = 8;  };
+template <> struct FftPlan<40>   { using type = Plan<40,   20, 20, 2>;        static constexpr int CS = 64, CC = 64; };
+template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        static constexpr int CS = 32, CC = 32; };
+template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int CS = 16, CC = 16; };
 
 }  // namespace mbs
 

@@ -159,13 +159,13 @@ static void report(const char* what, int M, double err) {
 template <int M>
 static void test_size() {
     using PL = typename FftPlan<M>::type;
-    constexpr int C = FftPlan<M>::C;
-    report("strided fwd", M, test_strided<PL, C, FFT_FWD>(2, 2, C + 5));
-    report("strided inv", M, test_strided<PL, C, FFT_INV>(1, 2, C + 5));
-    report("strided mid", M, test_strided<PL, C, FFT_MID>(1, 1, C + 3));
-    report("contig fwd", M, test_contig<PL, C, FFT_FWD>(2 * C + 3));
-    report("contig inv", M, test_contig<PL, C, FFT_INV>(C + 1));
-    report("contig mid", M, test_contig<PL, C, FFT_MID>(C + 2));
+    constexpr int CS = FftPlan<M>::CS, CC = FftPlan<M>::CC;
+    report("strided fwd", M, test_strided<PL, CS, FFT_FWD>(2, 2, CS + 5));
+    report("strided inv", M, test_strided<PL, CS, FFT_INV>(1, 2, CS + 5));
+    report("strided mid", M, test_strided<PL, CS, FFT_MID>(1, 1, CS + 3));
+    report("contig fwd", M, test_contig<PL, CC, FFT_FWD>(2 * CC + 3));
+    report("contig inv", M, test_contig<PL, CC, FFT_INV>(CC + 1));
+    report("contig mid", M, test_contig<PL, CC, FFT_MID>(CC + 2));
 }
 
 int main(int argc, char** argv) {

@@ -154,7 +154,8 @@ struct FusedParams {
 // FFT registry (fft_inst.cu compiled once per size, fft_registry.cu)
 struct FftEntry {
     int M;
-    int C;   // lines per tile
+    int CS;  // voxels per tile row of the strided sweeps
+    int CC;  // lines per tile of the contiguous sweeps
     cudaError_t (*strided)(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, int mode,
                            const int* done, int num_sms, int use_tma, cudaStream_t st);
     cudaError_t (*contig)(const cf* src, cf* dst, const ContigGeom& g, const SymbolParams& sp, const cf* tw, int mode,
