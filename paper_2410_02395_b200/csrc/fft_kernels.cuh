@@ -33,7 +33,11 @@ MBS_HD cf apply_symbol(cf v, float p2, const SymbolParams& sp) {
     const float dre = sp.A0 - sp.cr * p2;
     const float dim = sp.B0 - sp.ci * p2;
     if (sp.inverse) {
+#ifdef __CUDA_ARCH__
+        const float inv = __fdividef(sp.scale, dre * dre + dim * dim);   // 2 ulp; the bar is 1e-5 per operator
+#else
         const float inv = sp.scale / (dre * dre + dim * dim);
+#endif
         const cf g = make_float2(dre * inv, -dim * inv);
         return cmul(v, g);
     } else {

@@ -117,10 +117,12 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
     for (long long i = 0; i < n_mine; ++i) {
         const int s = (int)(i % NSTAGE);
         cf* tile = stage0 + (size_t)s * M * C;
-        if (tid == 0 && i + NSTAGE - 1 < n_mine) {
-            // the stage of tile i-1 is refilled: its store must have finished reading shared memory
-            tma_wait_read<0>();
-            issue_load(i + NSTAGE - 1);
+        if constexpr (NSTAGE < 3) {
+            if (tid == 0 && i + NSTAGE - 1 < n_mine) {
+                // the stage of tile i-1 is refilled: its store must have finished reading shared memory
+                tma_wait_read<0>();
+                issue_load(i + NSTAGE - 1);
+            }
         }
         mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
         int c0, c1, c2, ii0;
@@ -160,6 +162,14 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
 #pragma unroll
             for (int b = 0; b < NBOX; ++b) tma_store_3d(map, tile + (size_t)b * MB * C, c0, c1 + b * MB, c2);
             tma_commit();
+            if constexpr (NSTAGE >= 3) {
+                // refill the stage of tile i-1 with tile i+NSTAGE-1: only the store just committed may still be
+                // reading shared memory, so this never waits on a store in flight
+                if (i + NSTAGE - 1 < n_mine) {
+                    tma_wait_read<1>();
+                    issue_load(i + NSTAGE - 1);
+                }
+            }
         }
     }
     if (tid == 0) tma_wait_all();
