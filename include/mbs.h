@@ -68,6 +68,8 @@ enum mbs_option {
     MBS_OPT_USE_GRAPH = 2,      /* 1: replay each poll interval as a CUDA graph (default 1 for small grids)   */
     MBS_OPT_TMA = 4,            /* 1 (default): strided-axis FFT sweeps are fed by TMA box loads/stores through a
                                    shared-memory stage ring; 0: threads load/store the tiles themselves        */
+    MBS_OPT_LINE = 5,           /* 1 (default): first / last sweep as warp-line kernels (each warp owns whole lines of
+                                   the contiguous axis, no block barriers); 0: tile kernels with in-CTA edge terms  */
     MBS_OPT_PROFILE = 3         /* 1: bracket every kernel launch with CUDA events on the context's stream and
                                    accumulate per-kernel device time (mbs_get_kernel_stats); disables graphs   */
 };

@@ -82,6 +82,7 @@ struct mbs_ctx {
     int check_interval = 0;  // 0 = automatic
     int use_graph = -1;      // -1 = automatic
     int use_tma = 1;         // TMA-fed strided sweeps
+    int use_line = 1;        // warp-line first / last sweeps
 
     int profile = 0;
     Profiler prof;
@@ -227,11 +228,10 @@ static size_t layout_workspace(mbs_ctx* c, char* base) {
         const size_t n = corr_elems(g, ax);
         c->cx.buf[ax] = n ? (cf*)take(sizeof(cf) * n) : nullptr;
     }
-    for (int ax = 0; ax < 2; ++ax) {
+    for (int ax = 0; ax < 3; ++ax) {
         const size_t n = corr_elems(g, ax);
         c->ds.buf[ax] = n ? (cf*)take(sizeof(cf) * n) : nullptr;
     }
-    c->ds.buf[2] = nullptr;
     c->partials = (double*)take(sizeof(double) * MBS_MAX_PARTIALS * 5);
     c->ymask = (unsigned char*)take((size_t)(g.voxels / g.N[2]));
     return off;
@@ -404,6 +404,7 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
         case MBS_OPT_USE_GRAPH: c->use_graph = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_PROFILE: c->profile = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_TMA: c->use_tma = value ? 1 : 0; return MBS_OK;
+        case MBS_OPT_LINE: c->use_line = value ? 1 : 0; return MBS_OK;
         default: return fail(c, MBS_ERR_INVALID_ARG, "unknown option %d", option);
     }
 }
@@ -612,6 +613,36 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     }
     const int mask01 = (e0 ? 1 : 0) | (e1 ? 2 : 0);
     if (mask01) MBS_TRY(run_slabs(c, x, nullptr, true, mask01));                      // corr_0(x), corr_1(x)
+    if (c->use_line && e->line) {
+        // warp-line sweeps: corr_2(x) inside sweep 1; corr_2(d) through the compact buffers like axes 0 and 1
+        const int e2 = g.a[2] > 0 ? 1 : 0;
+        p.ds2 = c->ds.buf[2];
+        {
+            KernelScope ks(c, "line_sweep1", 4 * vb);
+            MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S1, done, c->num_sms, c->stream));
+        }
+        MBS_TRY(run_middle_sweeps(c, c->u, 1, true));
+        const int nb5 = e->line_blocks(LINE_S5, g.t, p.n_lines, c->num_sms);
+        if (nb5 < 1) return fail(c, MBS_ERR_CUDA, "line sweep: occupancy query failed");
+        const int mask = mask01 | (e2 ? 4 : 0);
+        p.slot0 = 0; p.n_total = nb5; p.finish = mask ? 0 : 1;
+        {
+            KernelScope ks(c, "line_sweep5", 4 * vb);
+            MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S5, done, c->num_sms, c->stream));
+        }
+        if (mask) {
+            MBS_TRY(run_slabs(c, nullptr, nullptr, true, mask, true));                // corr_d(d) from the compact d
+            FixupParams f{};
+            f.x = x; f.u = c->u; f.cx0 = c->cx.buf[0]; f.cx1 = c->cx.buf[1]; f.cx2 = c->cx.buf[2];
+            f.e0 = e0; f.e1 = e1; f.e2 = e2; f.alpha = (float)c->alpha;
+            f.partials = c->partials; f.slot0 = nb5; f.reduce_mode = RED_RESIDUAL; f.state = c->state; f.hist = c->hist_dev;
+            f.check_done = 1;
+            const double vox = (double)corr_elems(g, 0) + (double)corr_elems(g, 1) + (double)corr_elems(g, 2);
+            KernelScope ks(c, "fixup_slab_voxels", 32.0 * vox);
+            MBS_CUDA(c, launch_fixup(g, f, fixup_blocks(g, e0, e1, e2, c->num_sms), c->stream));
+        }
+        return MBS_OK;
+    }
     {
         KernelScope ks(c, "fused_sweep1", 4 * vb);                                    // reads x, B_diag, y; writes u
         MBS_CUDA(c, e->fused(p, c->tw_dev[2], FUSED_S1, done, c->num_sms, c->stream));
@@ -627,12 +658,13 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     if (mask01) {
         MBS_TRY(run_slabs(c, nullptr, nullptr, true, mask01, true));                  // corr_0(d), corr_1(d) from the compact d
         FixupParams f{};
-        f.x = x; f.u = c->u; f.cx0 = c->cx.buf[0]; f.cx1 = c->cx.buf[1]; f.e0 = e0; f.e1 = e1; f.alpha = (float)c->alpha;
+        f.x = x; f.u = c->u; f.cx0 = c->cx.buf[0]; f.cx1 = c->cx.buf[1]; f.cx2 = nullptr; f.e0 = e0; f.e1 = e1; f.e2 = 0;
+        f.alpha = (float)c->alpha;
         f.partials = c->partials; f.slot0 = nb5; f.reduce_mode = RED_RESIDUAL; f.state = c->state; f.hist = c->hist_dev;
         f.check_done = 1;
         const double rows = (double)corr_elems(g, 0) + (double)corr_elems(g, 1);
         KernelScope ks(c, "fixup_slab_rows", 40.0 * rows);
-        MBS_CUDA(c, launch_fixup(g, f, fixup_blocks(g, e0, e1, c->num_sms), c->stream));
+        MBS_CUDA(c, launch_fixup(g, f, fixup_blocks(g, e0, e1, 0, c->num_sms), c->stream));
     }
     return MBS_OK;
 }

@@ -304,4 +304,79 @@ MBS_DEV void fft_line_forward(cf (&v)[PL::P], cf* tile, const int c, const int j
     });
 }
 
+// ---------------------------------------------------------------------------------------------
+// Warp-local variant: the T <= 32 threads of a line are lanes of ONE warp, so the exchanges need only
+// __syncwarp and every warp runs its lines independently of the rest of the CTA.  `line` is the line's
+// private scratch of line_scratch_elems<PL>() elements; point i lives at i + (i >> 4) (one pad element per
+// 16), which makes both the scatter of a pass (stride R per lane) and the unit-stride read-back
+// conflict-free.  Device only.
+// ---------------------------------------------------------------------------------------------
+#ifdef __CUDACC__
+template <class PL>
+constexpr int line_scratch_elems() { return PL::M + PL::M / 16 + 1; }
+
+MBS_DEV int pad16(int i) { return i + (i >> 4); }
+
+template <class PL>
+MBS_DEV void fft_line_forward_warp(cf (&v)[PL::P], cf* line, const int jt, const cf* MBS_RESTRICT tw) {
+    constexpr int M = PL::M, P = PL::P, T = PL::T;
+    static_assert(T <= 32, "a line must fit in one warp");
+    static_for<0, PL::NPASS>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int R = PL::radix(i);
+        constexpr int Ns = PL::ns(i);
+        constexpr int NB = P / R;
+        constexpr bool last = (i == PL::NPASS - 1);
+        if constexpr (i > 0) {
+            static_for<0, NB>([&](auto bc) {
+                constexpr int b = decltype(bc)::value;
+                const int j = jt + b * T;
+                const int k = j % Ns;
+                const int step = k * (M / (Ns * R));
+                static_for<1, R>([&](auto rc) {
+                    constexpr int r = decltype(rc)::value;
+                    v[b + r * NB] = cmul(v[b + r * NB], tw[r * step]);
+                });
+            });
+        }
+        static_for<0, NB>([&](auto bc) {
+            constexpr int b = decltype(bc)::value;
+            Dft<R, b, NB, P>::run(v);
+        });
+        if constexpr (!last) {
+            static_for<0, NB>([&](auto bc) {
+                constexpr int b = decltype(bc)::value;
+                const int j = jt + b * T;
+                const int k = j % Ns;
+                const int j0 = (j - k) * R + k;
+                static_for<0, R>([&](auto rc) {
+                    constexpr int r = decltype(rc)::value;
+                    constexpr int src = b + NB * Dft<R, 0, 1, R>::slot(r);
+                    line[pad16(j0 + r * Ns)] = v[src];
+                });
+            });
+            __syncwarp();
+            static_for<0, P>([&](auto mc) {
+                constexpr int m = decltype(mc)::value;
+                v[m] = line[pad16(jt + m * T)];
+            });
+            __syncwarp();
+        } else {
+            cf w[P];
+            static_for<0, NB>([&](auto bc) {
+                constexpr int b = decltype(bc)::value;
+                static_for<0, R>([&](auto rc) {
+                    constexpr int r = decltype(rc)::value;
+                    w[b + r * NB] = v[b + NB * Dft<R, 0, 1, R>::slot(r)];
+                });
+            });
+            static_for<0, P>([&](auto mc) {
+                constexpr int m = decltype(mc)::value;
+                v[m] = w[m];
+            });
+        }
+    });
+}
+#endif
+
 }  // namespace mbs

@@ -4,6 +4,7 @@
 #include "mbs_internal.h"
 #include "fused_kernels.cuh"
 #include "fft_tma.cuh"
+#include "line_kernels.cuh"
 
 #ifndef MBS_FFT_SIZE
 #error "compile with -DMBS_FFT_SIZE=<M>"
@@ -80,6 +81,20 @@ __global__ void __launch_bounds__(NTC) k_fused_staged(const FusedParams p, const
     if (done && *done) return;
     if constexpr (staged_ok() && (MODE == FUSED_S1 || MODE == FUSED_S5))
         fused_staged_body<PL, CC, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
+}
+
+// warp-line variant of the first / last sweep (line_kernels.cuh): 8 warps per CTA, each warp owns whole lines
+constexpr bool line_ok() { return PL::T <= 32 && 32 % PL::T == 0; }
+constexpr int LINE_WARPS = 8;
+// resident CTAs per SM the compiler must allow: sweep 1 keeps <= 85 registers (24 warps per SM); sweep 5 holds x and
+// B_diag of a line in registers across the FFT (<= 128 registers, 16 warps per SM)
+template <int MODE>
+__global__ void __launch_bounds__(LINE_WARPS * 32, MODE == LINE_S1 ? 3 : 2) k_line(const FusedParams p, const cf* __restrict__ tw,
+                                                                         const int* __restrict__ done) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ double red[32];
+    if (done && *done) return;
+    if constexpr (line_ok()) line_body<PL, LINE_WARPS, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
 }
 
 // Opt in to the dynamic shared memory a kernel needs and query its occupancy; cached per (kernel, size).
@@ -207,6 +222,50 @@ int fused_blocks_entry(int mode, int t, long long n_tiles, int num_sms) {
     return e == cudaSuccess ? nb : -1;
 }
 
+template <int MODE>
+cudaError_t line_grid(int t, long long n_lines, int num_sms, int* nb_out, size_t* smem_out) {
+    if constexpr (!line_ok()) {
+        return cudaErrorNotSupported;
+    } else {
+        const size_t smem = line_smem_bytes<PL, LINE_WARPS>(t);
+        int bps = 1;
+        cudaError_t e = prepare(k_line<MODE>, LINE_WARPS * 32, smem, &bps);
+        if (e != cudaSuccess) return e;
+        const long long units = (n_lines + (32 / PL::T) - 1) / (32 / PL::T);
+        long long nb = (long long)num_sms * bps;
+        const long long need = (units + LINE_WARPS - 1) / LINE_WARPS;
+        if (nb > need) nb = need;
+        if (nb > MBS_MAX_PARTIALS / 2) nb = MBS_MAX_PARTIALS / 2;
+        if (nb < 1) nb = 1;
+        *nb_out = (int)nb;
+        *smem_out = smem;
+        return cudaSuccess;
+    }
+}
+
+cudaError_t line_entry(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st) {
+    int nb = 1;
+    size_t smem = 0;
+    if (mode == LINE_S1) {
+        cudaError_t e = line_grid<LINE_S1>(p.t, p.n_lines, num_sms, &nb, &smem);
+        if (e != cudaSuccess) return e;
+        k_line<LINE_S1><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
+    } else {
+        cudaError_t e = line_grid<LINE_S5>(p.t, p.n_lines, num_sms, &nb, &smem);
+        if (e != cudaSuccess) return e;
+        k_line<LINE_S5><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
+    }
+    return cudaGetLastError();
+}
+
+int line_blocks_entry(int mode, int t, long long n_lines, int num_sms) {
+    int nb = 1;
+    size_t smem = 0;
+    cudaError_t e = (mode == LINE_S1) ? line_grid<LINE_S1>(t, n_lines, num_sms, &nb, &smem)
+                                      : line_grid<LINE_S5>(t, n_lines, num_sms, &nb, &smem);
+    return e == cudaSuccess ? nb : -1;
+}
+
 cudaError_t strided_entry(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, int mode,
                           const int* done, int num_sms, int use_tma, cudaStream_t st) {
     // TMA needs 16-byte multiples for the global strides (inner even) and a 16-byte aligned base
@@ -237,7 +296,8 @@ cudaError_t contig_entry(const cf* src, cf* dst, const ContigGeom& g, const Symb
 
 #define MBS_CAT2(a, b) a##b
 #define MBS_CAT(a, b) MBS_CAT2(a, b)
-extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {MBS_FFT_SIZE, CS, CC, strided_entry, contig_entry, fused_entry,
-                                                                    fused_blocks_entry};
+extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {
+    MBS_FFT_SIZE, CS, CC, strided_entry, contig_entry, fused_entry, fused_blocks_entry,
+    line_ok() ? line_entry : nullptr, line_ok() ? line_blocks_entry : nullptr};
 
 }  // namespace mbs

@@ -448,7 +448,9 @@ __device__ __forceinline__ void fused_staged_body(const FusedParams& p, const cf
         if constexpr (MODE == FUSED_S5) {
             static_for<0, P>([&](auto mc) { v[decltype(mc)::value] = cswap(v[decltype(mc)::value]); });
         }
+#ifndef MBS_DBG_NOFFT
         fft_line_forward<PL, 1, LS>(v, tile, c_, jt, tw);
+#endif
         if constexpr (MODE == FUSED_S5) {
             static_for<0, P>([&](auto mc) { v[decltype(mc)::value] = cswap(v[decltype(mc)::value]); });
         }

@@ -371,6 +371,13 @@ __global__ void __launch_bounds__(PW_THREADS) k_fixup(const GridDesc g, const Fi
 #pragma unroll
             for (int v = 0; v < VEC; ++v) r[v] = csub(r[v], cc[v]);
         }
+        if (p.e2) {
+#pragma unroll
+            for (int v = 0; v < VEC; ++v) {
+                const int q2 = edge_slot(i2 + v, g.M[2], t);
+                if (q2 >= 0) r[v] = csub(r[v], p.cx2[((long long)i0 * g.N[1] + i1) * (g.S[2] * 2 * t) + q2]);
+            }
+        }
 #pragma unroll
         for (int v = 0; v < VEC; ++v) {
             acc += r[v].x * r[v].x + r[v].y * r[v].y;
@@ -378,16 +385,40 @@ __global__ void __launch_bounds__(PW_THREADS) k_fixup(const GridDesc g, const Fi
         }
         store_vec<VEC>(p.x + idx, xv);
     }
+    if (p.e2) {
+        // set C: the 2t edge points of every line on the rows that are in no slab of axis 0 or 1
+        const int E2 = g.S[2] * 2 * t;
+        const int w0 = p.e0 ? g.M[0] - 2 * t : g.M[0], w1 = p.e1 ? g.M[1] - 2 * t : g.M[1];
+        const long long n0 = (long long)g.S[0] * w0, n1 = (long long)g.S[1] * w1;
+        const long long n_items = n0 * n1 * E2;
+        for (long long item = (long long)blockIdx.x * PW_THREADS + threadIdx.x; item < n_items;
+             item += (long long)gridDim.x * PW_THREADS) {
+            const int q2 = (int)(item % E2);
+            const long long rr = item / E2;
+            const int k1 = (int)(rr % n1), k0 = (int)(rr / n1);
+            const int s0 = k0 / w0, s1 = k1 / w1;
+            const int i0 = s0 * g.M[0] + (p.e0 ? t : 0) + (k0 - s0 * w0);
+            const int i1 = s1 * g.M[1] + (p.e1 ? t : 0) + (k1 - s1 * w1);
+            const int i2 = edge_index(q2, g.M[2], t);
+            const long long row = (long long)i0 * g.N[1] + i1;
+            const long long idx = row * g.N[2] + i2;
+            const cf r = csub(p.u[idx], p.cx2[row * E2 + q2]);
+            const cf xv = p.x[idx];
+            acc += r.x * r.x + r.y * r.y;
+            p.x[idx] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
+        }
+    }
     const double bs = block_sum((double)acc, red);
     grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, 1, p.reduce_mode, p.state, p.hist, red);
 }
 
-int fixup_blocks(const GridDesc& g, int e0, int e1, int num_sms) {
+int fixup_blocks(const GridDesc& g, int e0, int e1, int e2, int num_sms) {
     const int vec = (g.N[2] % 2 == 0) ? 2 : 1;
     const int chunk_len = PW_THREADS * vec;
     const long long nchunks = (g.N[2] + chunk_len - 1) / chunk_len;
     const long long nE0 = e0 ? g.S[0] * 2 * g.t : 0, nE1 = e1 ? g.S[1] * 2 * g.t : 0;
-    const long long n_work = (nE0 * g.N[1] + (g.N[0] - nE0) * nE1) * nchunks;
+    long long n_work = (nE0 * g.N[1] + (g.N[0] - nE0) * nE1) * nchunks;
+    if (e2) n_work += ((g.N[0] - nE0) * (g.N[1] - nE1) * g.S[2] * 2 * g.t + PW_THREADS - 1) / PW_THREADS;
     long long nb = (long long)num_sms * 8;
     if (nb > MBS_MAX_PARTIALS / 2) nb = MBS_MAX_PARTIALS / 2;
     if (nb > n_work) nb = n_work;

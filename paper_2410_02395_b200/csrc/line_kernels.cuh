@@ -1,0 +1,185 @@
+// line_kernels.cuh -- warp-line variant of the first and last sweep of one iteration of Eq. (6).
+//
+// The T <= 32 threads that own one line of the contiguous axis are lanes of a single warp.  Each warp loads its
+// line(s) straight from global memory in the FFT's own register layout (thread jt holds points jt + m*T, so
+// every load/store instruction of a warp is one contiguous run), applies the scattering operator on the fly,
+// runs the FFT with warp-local exchanges through a private padded scratch line (__syncwarp only) and stores
+// the result.  No block-level barrier exists inside the loop: the 16-24 resident warps of an SM drift apart and
+// hide each other's HBM, shared-memory and pipeline latencies.
+//
+//   LINE_S1 : u = B_diag x + y_vec - corr_0(x) - corr_1(x) - corr_2(x), forward FFT         (a1, a2, a3)
+//             corr_0, corr_1 come from the compact buffers of the slab kernel; corr_2 (wrap-around C_ss and
+//             transfer A_{s,s+-1} along the line) is evaluated by the lanes that hold the 2t edge
+//             points from the edge points of the own and the neighbouring line, read in place.
+//   LINE_S5 : inverse FFT, d = x - u', r_part = B_diag d; every voxel outside all edge slabs is finished here
+//             (|r|^2, x -= alpha r: a6-a9); at slab voxels (rows in a slab of axis 0/1, or one of the 2t edge
+//             points of the line) it stores d to the compact buffers and r_part in place into u, and the
+//             fix-up kernels (kernels.cu) complete them.
+#pragma once
+#include "fft_kernels.cuh"
+#include "reduce.cuh"
+
+namespace mbs {
+
+template <class PL, int NWARP>
+constexpr size_t line_smem_bytes(int t) {
+    return sizeof(cf) * (size_t)(PL::M + NWARP * (32 / PL::T) * line_scratch_elems<PL>()) + sizeof(float) * (size_t)(t * t) + 16;
+}
+
+__device__ __forceinline__ int line_edge_slot(int i, int M, int t) {   // as fused_edge_slot: s*2t + e, or -1
+    const int s = i / M, e = i - s * M;
+    if (e < t) return s * 2 * t + e;
+    if (e >= M - t) return s * 2 * t + t + (e - (M - t));
+    return -1;
+}
+
+// corr_2(x) at edge point `pidx` of line (row, seg): c * sum_q K (x_nb[q] - x_own[q])   (P:124-128 with P:106)
+//   last  t points (a = pidx - (M-t)): K[a][q], own/nb = FIRST t points of this segment / of segment seg+1
+//   first t points (b = pidx):         K[q][b], own/nb = LAST  t points of this segment / of segment seg-1
+template <int M>
+__device__ __forceinline__ cf line_corr2_x(const FusedParams& p, const float* Ks, const long long grow, const int seg,
+                                           const int pidx) {
+    const int t = p.t;
+    const bool last = pidx >= M - t;
+    const int k = last ? pidx - (M - t) : pidx;
+    int nb = last ? seg + 1 : seg - 1;
+    bool has_nb = true;
+    if (nb < 0 || nb >= p.S2) {
+        if (p.per2) nb = (nb + p.S2) % p.S2;
+        else has_nb = false;
+    }
+    const cf* own = p.x + grow + (long long)seg * M + (last ? 0 : M - t);
+    const cf* nbp = p.x + grow + (long long)nb * M + (last ? 0 : M - t);
+    float sr = 0.f, si = 0.f;
+    for (int q = 0; q < t; ++q) {
+        const float kk = last ? Ks[k * t + q] : Ks[q * t + k];
+        cf dv = own[q];
+        dv = make_float2(-dv.x, -dv.y);
+        if (has_nb) {
+            const cf nv = nbp[q];
+            dv = make_float2(nv.x + dv.x, nv.y + dv.y);
+        }
+        sr = fmaf(kk, dv.x, sr);
+        si = fmaf(kk, dv.y, si);
+    }
+    return cmul(p.c, make_float2(sr, si));
+}
+
+template <class PL, int NWARP, int MODE>
+__device__ __forceinline__ void line_body(const FusedParams& p, const cf* __restrict__ tw_global, cf* smem, double* red) {
+    constexpr int M = PL::M, P = PL::P, T = PL::T, NT = NWARP * 32;
+    static_assert(T <= 32 && 32 % T == 0, "a line must fit in one warp");
+    constexpr int LW = 32 / T;                        // lines per warp
+    constexpr int LSE = line_scratch_elems<PL>();
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int t = p.t, t2 = 2 * p.t;
+    cf* tw = smem;
+    cf* scratch = tw + M + (warp * LW + lane / T) * LSE;
+    float* Ks = reinterpret_cast<float*>(tw + M + NWARP * LW * LSE);
+    for (int i = tid; i < M; i += NT) tw[i] = tw_global[i];
+    if (p.a2) for (int i = tid; i < t * t; i += NT) Ks[i] = p.Kh[i];
+    __syncthreads();
+    const int jt = lane % T, lsub = lane / T;
+    const unsigned n_lines = (unsigned)p.n_lines;
+    const unsigned n_units = (n_lines + LW - 1) / LW;
+    float acc = 0.f;
+    for (unsigned unit = blockIdx.x * NWARP + warp; unit < n_units; unit += gridDim.x * NWARP) {
+        const unsigned line = unit * LW + lsub;
+        const bool valid = line < n_lines;
+        const unsigned row = line / (unsigned)p.S2;
+        const int seg = (int)(line - row * (unsigned)p.S2);
+        const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
+        long long o0 = -1, o1 = -1;                   // compact row offsets of the axis-0 / axis-1 slabs
+        if (valid && p.e0) {
+            const int q = line_edge_slot(i0, p.M0, t);
+            if (q >= 0) o0 = ((long long)q * p.N1 + i1) * p.N2 + (long long)seg * M;
+        }
+        if (valid && p.e1) {
+            const int q = line_edge_slot(i1, p.M1, t);
+            if (q >= 0) o1 = ((long long)i0 * (p.S1 * t2) + q) * p.N2 + (long long)seg * M;
+        }
+        const long long gl = (long long)line * M;
+        const long long grow = (long long)row * p.N2;
+        cf v[P];
+        if constexpr (MODE == LINE_S1) {
+            const bool has_y = valid && p.y != nullptr && (p.ymask == nullptr || p.ymask[row] != 0);
+            static_for<0, P>([&](auto mc) {
+                constexpr int m = decltype(mc)::value;
+                const int pidx = jt + m * T;
+                v[m] = valid ? cmul(p.bdiag[gl + pidx], p.x[gl + pidx]) : make_float2(0.f, 0.f);
+            });
+            if (has_y) {
+                static_for<0, P>([&](auto mc) {
+                    constexpr int m = decltype(mc)::value;
+                    v[m] = cadd(v[m], cmul(p.ysc, p.y[gl + jt + m * T]));
+                });
+            }
+            if (o0 >= 0) {
+                static_for<0, P>([&](auto mc) {
+                    constexpr int m = decltype(mc)::value;
+                    v[m] = csub(v[m], p.cx0[o0 + jt + m * T]);
+                });
+            }
+            if (o1 >= 0) {
+                static_for<0, P>([&](auto mc) {
+                    constexpr int m = decltype(mc)::value;
+                    v[m] = csub(v[m], p.cx1[o1 + jt + m * T]);
+                });
+            }
+            if (p.a2 && valid) {
+                static_for<0, P>([&](auto mc) {
+                    constexpr int m = decltype(mc)::value;
+                    const int pidx = jt + m * T;
+                    if (pidx < t || pidx >= M - t) v[m] = csub(v[m], line_corr2_x<M>(p, Ks, grow, seg, pidx));
+                });
+            }
+            fft_line_forward_warp<PL>(v, scratch, jt, tw);
+            if (valid) {
+                static_for<0, P>([&](auto mc) {
+                    constexpr int m = decltype(mc)::value;
+                    p.u[gl + jt + m * T] = v[m];
+                });
+            }
+        } else {
+            static_for<0, P>([&](auto mc) {
+                constexpr int m = decltype(mc)::value;
+                v[m] = valid ? cswap(p.u[gl + jt + m * T]) : make_float2(0.f, 0.f);
+            });
+            // x and B_diag of the line are requested before the butterflies, so their HBM latency is covered
+            cf xr[P], br[P];
+            static_for<0, P>([&](auto mc) {
+                constexpr int m = decltype(mc)::value;
+                xr[m] = valid ? p.x[gl + jt + m * T] : make_float2(0.f, 0.f);
+                br[m] = valid ? p.bdiag[gl + jt + m * T] : make_float2(0.f, 0.f);
+            });
+            fft_line_forward_warp<PL>(v, scratch, jt, tw);
+            if (valid) {
+                const bool slab_row = (o0 >= 0) || (o1 >= 0);
+                const long long o2 = (long long)row * (p.S2 * t2) + (long long)seg * t2;
+                static_for<0, P>([&](auto mc) {
+                    constexpr int m = decltype(mc)::value;
+                    const int pidx = jt + m * T;
+                    const cf xv = xr[m];
+                    const cf d = csub(xv, cswap(v[m]));
+                    const cf r = cmul(br[m], d);
+                    const bool edge2 = p.a2 && (pidx < t || pidx >= M - t);
+                    if (!slab_row && !edge2) {
+                        acc += r.x * r.x + r.y * r.y;
+                        p.x[gl + pidx] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
+                    } else {
+                        if (o0 >= 0) p.ds0[o0 + pidx] = d;
+                        if (o1 >= 0) p.ds1[o1 + pidx] = d;
+                        if (edge2) p.ds2[o2 + (pidx < t ? pidx : pidx - (M - t2))] = d;
+                        p.u[gl + pidx] = r;
+                    }
+                });
+            }
+        }
+    }
+    if constexpr (MODE == LINE_S5) {
+        const double bs = block_sum((double)acc, red);
+        grid_reduce_finish(bs, p.partials, p.slot0, p.n_total, p.finish, p.reduce_mode, p.state, p.hist, red);
+    }
+}
+
+}  // namespace mbs

@@ -87,7 +87,8 @@ struct FixupParams {
     const cf* u;       // r_part on the slab rows
     const cf* cx0;     // corr_0(d), corr_1(d), compact
     const cf* cx1;
-    int e0, e1;
+    const cf* cx2;     // corr_2(d), compact [N0*N1][S2*2t] (warp-line path; else nullptr)
+    int e0, e1, e2;
     float alpha;
     double* partials;
     int slot0;         // first partial slot of this launch; slots below hold the fused sweep's partials
@@ -100,7 +101,7 @@ struct FixupParams {
 // launchers implemented in kernels.cu
 cudaError_t launch_pointwise(const GridDesc& g, const PointwiseParams& p, int num_sms, cudaStream_t st);
 cudaError_t launch_slab(const GridDesc& g, const SlabParams& p, cudaStream_t st);
-int fixup_blocks(const GridDesc& g, int e0, int e1, int num_sms);
+int fixup_blocks(const GridDesc& g, int e0, int e1, int e2, int num_sms);
 cudaError_t launch_fixup(const GridDesc& g, const FixupParams& p, int nblocks, cudaStream_t st);
 cudaError_t launch_row_mask(const cf* y, unsigned char* mask, long long rows, int N2, cudaStream_t st);
 cudaError_t launch_scale_copy(const cf* in, cf* out, cf scale, long long n, cudaStream_t st);
@@ -121,6 +122,7 @@ cudaError_t launch_setup(const GridDesc& g, const SetupParams& p, int pass, doub
 
 // fused first / last sweep along the contiguous axis (fused_kernels.cuh)
 enum FusedMode { FUSED_S1 = 0, FUSED_S5 = 1, FUSED_1D = 2 };
+enum LineMode { LINE_S1 = 0, LINE_S5 = 1 };   // warp-line variant (line_kernels.cuh)
 
 struct FusedParams {
     cf* x;               // iterate: read by S1; read and updated in place by S5 / 1D
@@ -138,6 +140,7 @@ struct FusedParams {
     const cf* cx1;       // S1: corr_1(x), compact [N0][S1*2t][N2]
     cf* ds0;             // S5: d at the axis-0 slab rows, same layouts
     cf* ds1;
+    cf* ds2;             // warp-line S5: d at the 2t edge points of every line, compact [N0*N1][S2*2t]
     const float* Kh;     // K_t / h^2, t x t row-major
     cf c;                // scale factor of Eq. (9)
     float alpha;
@@ -163,6 +166,9 @@ struct FftEntry {
     // fused sweep (FusedMode); *blocks_out = grid size used (number of residual partials written)
     cudaError_t (*fused)(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st);
     int (*fused_blocks)(int mode, int t, long long n_tiles, int num_sms);
+    // warp-line variant of the first / last sweep (line_kernels.cuh); nullptr when a line does not fit in a warp
+    cudaError_t (*line)(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st);
+    int (*line_blocks)(int mode, int t, long long n_lines, int num_sms);
 };
 const FftEntry* fft_lookup(int M);
 

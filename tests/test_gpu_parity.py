@@ -95,15 +95,16 @@ ITERATION_CASES = OPERATOR_CASES + [
 ]
 
 
-@pytest.mark.parametrize("fused,tma", [(1, 1), (0, 1), (1, 0)])
+@pytest.mark.parametrize("fused,tma,line", [(1, 1, 1), (1, 1, 0), (0, 1, 1), (1, 0, 0)])
 @pytest.mark.parametrize("shape,S,W,t,periodic", ITERATION_CASES)
-def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma):
+def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line):
     """A few updates of Eq. (6) from a random start with a dense random source, fused sweeps and
     one-kernel-per-step path, against the oracle's iterates: every step of SURVEY 8(a) on every geometry."""
     import torch
     s, o, n = make_pair(B, orc, shape, S, W, t, periodic, seed=11)
     s.set_option(B.MBS_OPT_FUSED, fused)
     s.set_option(B.MBS_OPT_TMA, tma)
+    s.set_option(B.MBS_OPT_LINE, line)
     y = workloads.random_field(shape, 21)
     x0 = workloads.random_field(shape, 22)
     n_it = 6
