@@ -158,14 +158,16 @@ def workload_name(w):
         "x".join(map(str, w.boundary_width)))
 
 
-def dominant_kernel_traffic(name):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel class `name`, from the committed
-    ncu --set full capture (profiles/dram_traffic.json, written by hand from the capture named there)."""
+def dominant_kernel_traffic(name, voxels):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel class `name`: measured per voxel in the committed
+    ncu --set full capture (profiles/dram_traffic.json, from profiles/r01_ncu_full_summary.md, a smaller grid of the same
+    line lengths) and scaled to this workload's voxel count.  None when the kernel is not in the capture."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.json")
     if not os.path.exists(path):
         return None
     try:
-        return json.load(open(path)).get(name, {}).get("dram_bytes_per_launch")
+        per_voxel = json.load(open(path))["kernels"][name]["dram_bytes_per_voxel"]
+        return per_voxel * voxels
     except Exception:
         return None
 
@@ -242,7 +244,7 @@ def run_b200(args):
     info = s.info()
     alg_bytes_it = info["algorithmic_bytes_per_iteration"]
     roofline = {"bound": "hbm", "kernel": top["name"], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": dominant_kernel_traffic(top["name"]), "peak_kind": peak_kind,
+                "frac": achieved / peak, "traffic": dominant_kernel_traffic(top["name"], w.voxels), "peak_kind": peak_kind,
                 "algorithmic_bytes_per_launch": top_bytes, "avg_launch_ms": top_ms,
                 "share_of_step": top["total_ms"] / total_kernel_ms,
                 "whole_step": {"algorithmic_bytes_per_voxel_iteration": alg_bytes_it / w.voxels,
