@@ -172,6 +172,22 @@ def dominant_kernel_traffic(name, voxels):
         return None
 
 
+def max_over_ranks(ms, device):
+    """Device time of the timed region as the max over ranks (every rank gets it); identity without a process group."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(ms)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_throughput(voxels, steps, ms, world):
+    """Whole-job Gvoxel-iterations/s of `world` independent replicas that each did `steps` iterations in `ms`."""
+    return world * voxels * steps / (ms * 1e-3) / 1e9
+
+
 def run_b200(args):
     import torch
     import torch.distributed as dist
@@ -226,11 +242,8 @@ def run_b200(args):
     launches = s.info()["kernel_launches"] - launches0
     stats = s.kernel_stats()
     s.set_option(binding.MBS_OPT_PROFILE, 0)
-    if world > 1:
-        tms = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        ms = float(tms.item())
-    value = world * w.voxels * K / (ms * 1e-3) / 1e9
+    ms = max_over_ranks(ms, dev)
+    value = aggregate_throughput(w.voxels, K, ms, world)
 
     # roofline of the dominant kernel
     peak, peak_kind = peaks()

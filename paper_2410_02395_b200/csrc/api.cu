@@ -87,6 +87,14 @@ struct mbs_ctx {
     int profile = 0;
     Profiler prof;
 
+    // CUDA graph of one poll interval of iterations (small grids are launch-bound)
+    cudaGraphExec_t graph_exec = nullptr;
+    cudaStream_t cap_stream = nullptr;   // capture happens on a private stream (the caller's may be the default stream)
+    const void* graph_y = nullptr;
+    const void* graph_x = nullptr;
+    int graph_batch = 0, graph_fused = -1, graph_tma = -1, graph_line = -1;
+    int64_t launches_per_batch = 0;
+
     int64_t launches = 0;
     std::string err;
 };
@@ -366,6 +374,8 @@ extern "C" void mbs_destroy(mbs_ctx* c) {
     if (c->host_y) cudaFree(c->host_y);
     if (c->host_x) cudaFree(c->host_x);
     for (cudaEvent_t e : c->prof.pool) cudaEventDestroy(e);
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     delete c;
 }
 
@@ -738,6 +748,45 @@ static int ensure_history(mbs_ctx* c, int32_t max_iter) {
     return MBS_OK;
 }
 
+// Enqueue `batch` iterations: as individual launches, or (graphs on, not profiling) as one replay of a CUDA graph
+// captured from the same launches.  The graph is rebuilt when the arrays, the batch or the kernel options change.
+static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_graph) {
+    const bool graph_on = allow_graph && !c->profile &&
+                          (c->use_graph == 1 || (c->use_graph < 0 && c->g.voxels <= (1LL << 25)));
+    if (!graph_on) {
+        for (int i = 0; i < batch; ++i) MBS_TRY(run_iteration(c, y, x));
+        return MBS_OK;
+    }
+    const bool stale = !c->graph_exec || c->graph_y != y || c->graph_x != x || c->graph_batch != batch ||
+                       c->graph_fused != c->fused || c->graph_tma != c->use_tma || c->graph_line != c->use_line;
+    if (stale) {
+        if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
+        if (!c->cap_stream) MBS_CUDA(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
+        MBS_CUDA(c, cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal));
+        int rc = MBS_OK;
+        const int64_t launches0 = c->launches;
+        cudaStream_t user_stream = c->stream;
+        c->stream = c->cap_stream;                    // every launch site enqueues on c->stream
+        for (int i = 0; i < batch && rc == MBS_OK; ++i) rc = run_iteration(c, y, x);
+        c->stream = user_stream;
+        const int64_t captured = c->launches - launches0;
+        c->launches = launches0;                      // counted per replay below
+        cudaGraph_t graph = nullptr;
+        const cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
+        if (rc != MBS_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+        if (e != cudaSuccess) return fail(c, MBS_ERR_CUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+        const cudaError_t e2 = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e2 != cudaSuccess) { c->graph_exec = nullptr; return fail(c, MBS_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e2)); }
+        c->graph_y = y; c->graph_x = x; c->graph_batch = batch;
+        c->graph_fused = c->fused; c->graph_tma = c->use_tma; c->graph_line = c->use_line;
+        c->launches_per_batch = captured;
+    }
+    MBS_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));
+    c->launches += c->launches_per_batch;
+    return MBS_OK;
+}
+
 static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_iter, double* residual_history,
                         int32_t* n_iter) {
     if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
@@ -750,7 +799,7 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
 
     int interval = c->check_interval;
     if (interval <= 0) {
-        interval = (int)std::max<long long>(1, std::min<long long>(64, (4LL << 20) / std::max<long long>(1, c->g.voxels)));
+        interval = (int)std::max<long long>(1, std::min<long long>(64, (64LL << 20) / std::max<long long>(1, c->g.voxels)));
     }
     MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
     int enqueued = 0;
@@ -759,9 +808,12 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
     int final_done = 0;
     while (true) {
         // enqueue one batch, then look at the poll of the PREVIOUS batch (one batch of lookahead keeps the GPU busy)
-        const int batch = std::min(interval, max_iter - enqueued);
+        // the first batch is enqueued launch by launch (it also warms the per-kernel attribute caches); later batches
+        // replay a graph of a full interval: kernels past max_iter return at once on the device flag
+        const bool first = (enqueued == 0);
+        const int batch = first ? std::min(interval, max_iter - enqueued) : (enqueued < max_iter ? interval : 0);
         if (batch > 0 && !final_done) {
-            for (int i = 0; i < batch; ++i) MBS_TRY(run_iteration(c, y, x));
+            MBS_TRY(enqueue_batch(c, y, x, batch, !first));
             enqueued += batch;
             MBS_CUDA(c, cudaMemcpyAsync(&c->state_pinned[slot], c->state, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
             MBS_CUDA(c, cudaEventRecord(c->ev_poll[slot], c->stream));
