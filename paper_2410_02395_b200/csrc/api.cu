@@ -63,6 +63,7 @@ struct mbs_ctx {
     float* Kh_dev = nullptr;
     cf* tw_dev[3] = {nullptr, nullptr, nullptr};
     float* p2_dev[3] = {nullptr, nullptr, nullptr};
+    float* wtab_dev = nullptr;   // |p|^2 of the axes after the first one, per inner index of the kernel-multiply sweep
     const FftEntry* fft[3] = {nullptr, nullptr, nullptr};
     DevState* state_pinned = nullptr;  // 2 slots for polling
     cudaEvent_t ev_poll[2] = {nullptr, nullptr};
@@ -351,6 +352,31 @@ extern "C" int mbs_create(mbs_ctx** out, int ndim, const int64_t* shape, double 
             (e = cudaMemcpy(c->p2_dev[ax], p2.data(), sizeof(float) * M, cudaMemcpyHostToDevice)) != cudaSuccess)
             return cleanup_fail(MBS_ERR_CUDA, "cudaMemcpy(tables)", e);
     }
+    if (ndim >= 2) {
+        // per-line part of |p|^2 for the kernel-multiply sweep along the first axis (one float per inner index)
+        long long inner = 1;
+        for (int ax = c->first + 1; ax < 3; ++ax) inner *= g.N[ax];
+        std::vector<float> wt((size_t)inner);
+        std::vector<std::vector<double>> p2d(3);
+        for (int ax = c->first + 1; ax < 3; ++ax) {
+            const int M = g.M[ax];
+            p2d[ax].resize(M);
+            for (int n = 0; n < M; ++n) {
+                const int f = (n < (M + 1) / 2) ? n : n - M;
+                const double p = 2.0 * M_PI * (double)f / ((double)M * pixel_size);
+                p2d[ax][n] = (double)(float)(p * p);      // the same rounded values as the per-axis tables
+            }
+        }
+        for (long long ii = 0; ii < inner; ++ii) {
+            const int i2 = (int)(ii % g.N[2]);
+            float w = (float)p2d[2][i2 % g.M[2]];
+            if (c->first == 0) w += (float)p2d[1][(int)((ii / g.N[2]) % g.M[1])];
+            wt[(size_t)ii] = w;
+        }
+        if ((e = cudaMalloc(&c->wtab_dev, sizeof(float) * wt.size())) != cudaSuccess) return cleanup_fail(MBS_ERR_OOM, "cudaMalloc(wtab)", e);
+        if ((e = cudaMemcpy(c->wtab_dev, wt.data(), sizeof(float) * wt.size(), cudaMemcpyHostToDevice)) != cudaSuccess)
+            return cleanup_fail(MBS_ERR_CUDA, "cudaMemcpy(wtab)", e);
+    }
     c->ws_bytes = layout_workspace(c, nullptr);
     *out = c;
     return MBS_OK;
@@ -362,6 +388,7 @@ extern "C" void mbs_destroy(mbs_ctx* c) {
     if (c->state) cudaFree(c->state);
     if (c->hist_dev) cudaFree(c->hist_dev);
     if (c->Kh_dev) cudaFree(c->Kh_dev);
+    if (c->wtab_dev) cudaFree(c->wtab_dev);
     for (int ax = 0; ax < 3; ++ax) {
         if (c->tw_dev[ax]) cudaFree(c->tw_dev[ax]);
         if (c->p2_dev[ax]) cudaFree(c->p2_dev[ax]);
@@ -543,6 +570,7 @@ static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, b
         // line-invariant part of |p|^2 from the axes after `ax`
         if (ax == 0) { s2.tabA = c->p2_dev[1]; s2.Ma = g.M[1]; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
         else { s2.tabA = nullptr; s2.Ma = 1; s2.tabB = c->p2_dev[2]; s2.Mb = g.M[2]; s2.Nb = g.N[2]; }
+        if (ax == c->first) s2.wtab = c->wtab_dev;
     }
     static const char* names[2][3] = {{"fft_strided_fwd_ax0", "fft_strided_inv_ax0", "fft_strided_mid_ax0"},
                                       {"fft_strided_fwd_ax1", "fft_strided_inv_ax1", "fft_strided_mid_ax1"}};

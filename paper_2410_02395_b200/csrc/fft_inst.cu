@@ -88,8 +88,11 @@ constexpr bool line_ok() { return PL::T <= 32 && 32 % PL::T == 0; }
 constexpr int LINE_WARPS = 8;
 // resident CTAs per SM the compiler must allow: sweep 1 keeps <= 85 registers (24 warps per SM); sweep 5 holds x and
 // B_diag of a line in registers across the FFT (<= 128 registers, 16 warps per SM)
+#ifndef MBS_LINE_MINB_S1
+#define MBS_LINE_MINB_S1 3
+#endif
 template <int MODE>
-__global__ void __launch_bounds__(LINE_WARPS * 32, MODE == LINE_S1 ? 3 : 2) k_line(const FusedParams p, const cf* __restrict__ tw,
+__global__ void __launch_bounds__(LINE_WARPS * 32, MODE == LINE_S1 ? MBS_LINE_MINB_S1 : 2) k_line(const FusedParams p, const cf* __restrict__ tw,
                                                                          const int* __restrict__ done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];

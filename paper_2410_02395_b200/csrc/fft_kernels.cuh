@@ -27,6 +27,7 @@ struct SymbolParams {
     const float* tabA;       // p^2 table of the slower inner axis (period Ma), or nullptr
     const float* tabB;       // p^2 table of the faster inner axis (period Mb), or nullptr
     int Nb, Ma, Mb;          // inner index ii -> (ii / Nb) % Ma, (ii % Nb) % Mb
+    const float* wtab;       // optional: tabA[..] + tabB[..] tabulated per inner index ii (replaces the two lookups)
 };
 
 MBS_HD cf apply_symbol(cf v, float p2, const SymbolParams& sp) {

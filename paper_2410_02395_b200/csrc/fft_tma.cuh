@@ -90,19 +90,22 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
     __syncthreads();
     const int c = tid % C;
     const int jt = tid / C;
-    const long long first = blockIdx.x, step = gridDim.x;
-    const long long n_mine = first < g.n_tiles ? (g.n_tiles - first + step - 1) / step : 0;
+    // tile counters fit 32 bits (fewer than 2^31 voxels): keep the per-tile index arithmetic cheap
+    const unsigned first = blockIdx.x, step = gridDim.x, n_tiles = (unsigned)g.n_tiles;
+    const unsigned n_mine = first < n_tiles ? (n_tiles - first + step - 1) / step : 0;
+    const unsigned tiles_inner = (unsigned)g.tiles_inner, n_seg = (unsigned)g.n_seg;
 
-    auto coords = [&](long long i, int& c0, int& c1, int& c2, int& ii0) {
-        const long long tix = first + i * step;
-        const int ic = (int)(tix % g.tiles_inner);
-        const long long os = tix / g.tiles_inner;
-        c0 = 2 * ic * C;
-        c1 = (int)(os % g.n_seg) * M;
-        c2 = (int)(os / g.n_seg);
-        ii0 = ic * C;
+    auto coords = [&](unsigned i, int& c0, int& c1, int& c2, int& ii0) {
+        const unsigned tix = first + i * step;
+        const unsigned os = tix / tiles_inner;
+        const unsigned ic = tix - os * tiles_inner;
+        const unsigned o = os / n_seg;
+        c0 = (int)(2 * ic * C);
+        c1 = (int)(os - o * n_seg) * M;
+        c2 = (int)o;
+        ii0 = (int)(ic * C);
     };
-    auto issue_load = [&](long long i) {
+    auto issue_load = [&](unsigned i) {
         int c0, c1, c2, ii0;
         coords(i, c0, c1, c2, ii0);
         const int s = (int)(i % NSTAGE);
@@ -112,9 +115,14 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
             tma_load_3d(stage0 + (size_t)s * M * C + (size_t)b * MB * C, map, &full[s], c0, c1 + b * MB, c2);
     };
     if (tid == 0) {
-        for (long long i = 0; i < NSTAGE - 1 && i < n_mine; ++i) issue_load(i);
+        for (unsigned i = 0; i < NSTAGE - 1 && i < n_mine; ++i) issue_load(i);
     }
-    for (long long i = 0; i < n_mine; ++i) {
+    // |p|^2 of the transformed axis at this thread's points (kernel-multiply sweep)
+    float p2a[P];
+    if constexpr (MODE == FFT_MID) {
+        static_for<0, P>([&](auto mc) { p2a[decltype(mc)::value] = sp.tab_axis[jt + decltype(mc)::value * T]; });
+    }
+    for (unsigned i = 0; i < n_mine; ++i) {
         const int s = (int)(i % NSTAGE);
         cf* tile = stage0 + (size_t)s * M * C;
         if constexpr (NSTAGE < 3) {
@@ -140,12 +148,15 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
         if constexpr (MODE == FFT_MID) {
             const int ii = ii0 + c;
             float wline = 0.f;
-            if (sp.tabA) wline += sp.tabA[(ii / sp.Nb) % sp.Ma];
-            if (sp.tabB) wline += sp.tabB[(ii % sp.Nb) % sp.Mb];
+            if (sp.wtab) {
+                wline = ii < g.inner ? sp.wtab[ii] : 0.f;       // |p|^2 of the other axes, one value per line
+            } else {
+                if (sp.tabA) wline += sp.tabA[(ii / sp.Nb) % sp.Ma];
+                if (sp.tabB) wline += sp.tabB[(ii % sp.Nb) % sp.Mb];
+            }
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
-                const float p2 = sp.tab_axis[jt + m * T] + wline;
-                v[m] = cswap(apply_symbol(v[m], p2, sp));
+                v[m] = cswap(apply_symbol(v[m], p2a[m] + wline, sp));
             });
             fft_line_forward<PL, C, 1>(v, tile, c, jt, tw);
         }
