@@ -19,7 +19,7 @@ template <> struct FftPlan<1024> { using type = Plan<1024, 16, 16, 16, 4>;    st
 template <> struct FftPlan<40>   { using type = Plan<40,   20, 20, 2>;        static constexpr int CS = 64, CC = 64; };
 template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        static constexpr int CS = 32, CC = 32; };
 template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 32, CC = 16; };
 template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int CS = 16, CC = 16; };
 
 }  // namespace mbs
