@@ -668,7 +668,21 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
             KernelScope ks(c, "line_sweep5", 4 * vb);
             MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S5, done, c->num_sms, c->stream));
         }
-        if (mask) {
+        if (mask && slab_pass_supported(g.t)) {
+            // one pass per axis: corr_ax(d) from the compact d, applied in the same kernel; the last pass finishes
+            int slot = nb5, last_ax = (mask & 4) ? 2 : ((mask & 2) ? 1 : 0);
+            for (int ax = 0; ax < 3; ++ax) {
+                if (!((mask >> ax) & 1)) continue;
+                SlabPassParams sp{};
+                sp.ds = c->ds.buf[ax]; sp.u = c->u; sp.x = x; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
+                sp.e1 = e1; sp.e2 = e2; sp.alpha = (float)c->alpha; sp.partials = c->partials; sp.slot0 = slot;
+                sp.finish = (ax == last_ax) ? 1 : 0; sp.state = c->state; sp.hist = c->hist_dev;
+                static const char* names[3] = {"slab_pass_ax0", "slab_pass_ax1", "slab_pass_ax2"};
+                KernelScope ks(c, names[ax], 40.0 * (double)corr_elems(g, ax));
+                MBS_CUDA(c, launch_slab_pass(g, sp, c->stream));
+                slot += slab_pass_blocks(g, ax);
+            }
+        } else if (mask) {
             MBS_TRY(run_slabs(c, nullptr, nullptr, true, mask, true));                // corr_d(d) from the compact d
             FixupParams f{};
             f.x = x; f.u = c->u; f.cx0 = c->cx.buf[0]; f.cx1 = c->cx.buf[1]; f.cx2 = c->cx.buf[2];

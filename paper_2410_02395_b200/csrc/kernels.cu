@@ -233,6 +233,123 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab(const GridDesc g, const S
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// slab pass (fix-up of the warp-line last sweep): for one axis, corr_ax(d) from the compact d and its
+// application in the same kernel.  At each of the t edge voxels an item owns:
+//     r = u - corr_ax(d)          (u holds r_part = B_diag d, minus the corrections of the earlier axes)
+// and then either the voxel is also an edge point of a LATER axis (its pass will finish it): u = r; or this is
+// its last correction:  |r|^2 partial sum,  x <- x - alpha r        (a7-a9).
+// Passes run in axis order 0, 1, 2 on the stream; the last one finishes the reduction and the stop test.
+// ---------------------------------------------------------------------------------------------
+template <int TT>
+__global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, const SlabPassParams p, const long long outer,
+                                                            const long long inner, const long long n_items) {
+    __shared__ float Ks[TT * TT];
+    __shared__ double red[32];
+    if (p.state->done) return;
+    constexpr int t = TT;
+    for (int i = threadIdx.x; i < TT * TT; i += SLAB_THREADS) Ks[i] = p.Kh[i];
+    __syncthreads();
+    const int ax = p.axis;
+    const int S = g.S[ax], M = g.M[ax];
+    float acc = 0.f;
+    for (long long item = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x; item < n_items;
+         item += (long long)gridDim.x * SLAB_THREADS) {
+        const long long in_i = item % inner;
+        long long rest = item / inner;
+        const int side = (int)(rest % 2);
+        rest /= 2;
+        const int s = (int)(rest % S);
+        const long long o = rest / S;
+        int nb = side ? s + 1 : s - 1;
+        bool has_nb = true;
+        if (nb < 0 || nb >= S) {
+            if (g.per[ax]) nb = (nb + S) % S;
+            else has_nb = false;
+        }
+        // side 1 (last t points of s) reads the FIRST t points of s and s+1; side 0 reads the LAST t points
+        const long long own0 = ((o * S + s) * 2 * t + (side ? 0 : t)) * inner + in_i;
+        const long long nb0 = ((o * S + nb) * 2 * t + (side ? 0 : t)) * inner + in_i;
+        cf dv[TT];
+#pragma unroll
+        for (int q = 0; q < TT; ++q) {
+            const cf own = p.ds[own0 + q * inner];
+            cf nbv = make_float2(0.f, 0.f);
+            if (has_nb) nbv = p.ds[nb0 + q * inner];
+            dv[q] = make_float2(nbv.x - own.x, nbv.y - own.y);
+        }
+        // is the voxel an edge point of a later axis?  (constant over the t outputs of this item)
+        bool later = false;
+        long long vox0, vstride;                      // voxel index of output e: vox0 + e * vstride
+        const int ia0 = s * M + (side ? M - t : 0);
+        if (ax == 0) {
+            const int i1 = (int)(in_i / g.N[2]), i2 = (int)(in_i - (long long)i1 * g.N[2]);
+            later = (p.e1 && edge_slot(i1, g.M[1], t) >= 0) || (p.e2 && edge_slot(i2, g.M[2], t) >= 0);
+            vox0 = (long long)ia0 * inner + in_i;
+            vstride = inner;
+        } else if (ax == 1) {
+            later = p.e2 && edge_slot((int)in_i, g.M[2], t) >= 0;
+            vox0 = (o * g.N[1] + ia0) * inner + in_i;
+            vstride = inner;
+        } else {
+            vox0 = o * g.N[2] + ia0;
+            vstride = 1;
+        }
+#pragma unroll
+        for (int e = 0; e < TT; ++e) {
+            float sr = 0.f, si = 0.f;
+#pragma unroll
+            for (int q = 0; q < TT; ++q) {
+                const float k = side ? Ks[e * TT + q] : Ks[q * TT + e];
+                sr = fmaf(k, dv[q].x, sr);
+                si = fmaf(k, dv[q].y, si);
+            }
+            const cf corr = cmul(p.c, make_float2(sr, si));
+            const long long vox = vox0 + e * vstride;
+            const cf uu = p.u[vox];
+            const cf r = make_float2(uu.x - corr.x, uu.y - corr.y);
+            if (later) {
+                p.u[vox] = r;
+            } else {
+                const cf xv = p.x[vox];
+                acc += r.x * r.x + r.y * r.y;
+                p.x[vox] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
+            }
+        }
+    }
+    const double bs = block_sum((double)acc, red);
+    grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, p.finish, RED_RESIDUAL, p.state, p.hist, red);
+}
+
+int slab_pass_blocks(const GridDesc& g, int ax) {
+    long long outer = 1, inner = 1;
+    for (int d = 0; d < ax; ++d) outer *= g.N[d];
+    for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
+    const long long n_items = outer * g.S[ax] * 2 * inner;
+    long long nb = (n_items + SLAB_THREADS - 1) / SLAB_THREADS;
+    if (nb > 1024) nb = 1024;
+    return (int)(nb < 1 ? 1 : nb);
+}
+
+bool slab_pass_supported(int t) { return t == 2 || t == 4 || t == 8 || t == 16; }
+
+cudaError_t launch_slab_pass(const GridDesc& g, const SlabPassParams& p, cudaStream_t st) {
+    const int ax = p.axis;
+    long long outer = 1, inner = 1;
+    for (int d = 0; d < ax; ++d) outer *= g.N[d];
+    for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
+    const long long n_items = outer * g.S[ax] * 2 * inner;
+    const int nb = slab_pass_blocks(g, ax);
+    switch (g.t) {
+        case 2: k_slab_pass<2><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
+        case 4: k_slab_pass<4><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
+        case 8: k_slab_pass<8><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
+        case 16: k_slab_pass<16><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
+        default: return cudaErrorNotSupported;
+    }
+    return cudaGetLastError();
+}
+
 // generic t (any value): one thread per output element
 __global__ void __launch_bounds__(SLAB_THREADS) k_slab_generic(const GridDesc g, const SlabParams p,
                                                                const long long outer, const long long inner,

@@ -101,6 +101,25 @@ struct FixupParams {
 // launchers implemented in kernels.cu
 cudaError_t launch_pointwise(const GridDesc& g, const PointwiseParams& p, int num_sms, cudaStream_t st);
 cudaError_t launch_slab(const GridDesc& g, const SlabParams& p, cudaStream_t st);
+// slab pass of one axis (kernels.cu: k_slab_pass): corr_ax(d) from the compact d, applied to u / x in the same kernel
+struct SlabPassParams {
+    const cf* ds;      // compact d of this axis, [outer][S*2t][inner]
+    cf* u;             // r_part minus the corrections of the earlier axes, at the slab voxels
+    cf* x;
+    const float* Kh;
+    cf c;
+    int axis;
+    int e1, e2;        // axes 1 / 2 have edge corrections (later passes exist)
+    float alpha;
+    double* partials;
+    int slot0;         // first partial slot of this launch
+    int finish;        // 1: this is the last pass: add all partials [0, slot0 + grid) and finish the iteration
+    DevState* state;
+    double* hist;
+};
+int slab_pass_blocks(const GridDesc& g, int ax);
+bool slab_pass_supported(int t);
+cudaError_t launch_slab_pass(const GridDesc& g, const SlabPassParams& p, cudaStream_t st);
 int fixup_blocks(const GridDesc& g, int e0, int e1, int e2, int num_sms);
 cudaError_t launch_fixup(const GridDesc& g, const FixupParams& p, int nblocks, cudaStream_t st);
 cudaError_t launch_row_mask(const cf* y, unsigned char* mask, long long rows, int N2, cudaStream_t st);
