@@ -36,10 +36,11 @@ __device__ __forceinline__ int line_edge_slot(int i, int M, int t) {   // as fus
 // corr_2(x) at edge point `pidx` of line (row, seg): c * sum_q K (x_nb[q] - x_own[q])   (P:124-128 with P:106)
 //   last  t points (a = pidx - (M-t)): K[a][q], own/nb = FIRST t points of this segment / of segment seg+1
 //   first t points (b = pidx):         K[q][b], own/nb = LAST  t points of this segment / of segment seg-1
-template <int M>
-__device__ __forceinline__ cf line_corr2_x(const FusedParams& p, const float* Ks, const long long grow, const int seg,
-                                           const int pidx) {
-    const int t = p.t;
+// TT > 0: t known at compile time (all 2t loads are issued before the first use); TT = 0: any t.
+template <int M, int TT>
+__device__ __forceinline__ cf line_corr2_x_t(const FusedParams& p, const float* Ks, const long long grow, const int seg,
+                                             const int pidx) {
+    const int t = TT > 0 ? TT : p.t;
     const bool last = pidx >= M - t;
     const int k = last ? pidx - (M - t) : pidx;
     int nb = last ? seg + 1 : seg - 1;
@@ -51,18 +52,41 @@ __device__ __forceinline__ cf line_corr2_x(const FusedParams& p, const float* Ks
     const cf* own = p.x + grow + (long long)seg * M + (last ? 0 : M - t);
     const cf* nbp = p.x + grow + (long long)nb * M + (last ? 0 : M - t);
     float sr = 0.f, si = 0.f;
-    for (int q = 0; q < t; ++q) {
-        const float kk = last ? Ks[k * t + q] : Ks[q * t + k];
-        cf dv = own[q];
-        dv = make_float2(-dv.x, -dv.y);
-        if (has_nb) {
-            const cf nv = nbp[q];
-            dv = make_float2(nv.x + dv.x, nv.y + dv.y);
+    if constexpr (TT > 0) {
+        cf ov[TT], nv[TT];
+#pragma unroll
+        for (int q = 0; q < TT; ++q) {
+            ov[q] = own[q];
+            nv[q] = has_nb ? nbp[q] : make_float2(0.f, 0.f);
         }
-        sr = fmaf(kk, dv.x, sr);
-        si = fmaf(kk, dv.y, si);
+#pragma unroll
+        for (int q = 0; q < TT; ++q) {
+            const float kk = last ? Ks[k * TT + q] : Ks[q * TT + k];
+            sr = fmaf(kk, nv[q].x - ov[q].x, sr);
+            si = fmaf(kk, nv[q].y - ov[q].y, si);
+        }
+    } else {
+        for (int q = 0; q < t; ++q) {
+            const float kk = last ? Ks[k * t + q] : Ks[q * t + k];
+            cf dv = own[q];
+            dv = make_float2(-dv.x, -dv.y);
+            if (has_nb) {
+                const cf nv = nbp[q];
+                dv = make_float2(nv.x + dv.x, nv.y + dv.y);
+            }
+            sr = fmaf(kk, dv.x, sr);
+            si = fmaf(kk, dv.y, si);
+        }
     }
     return cmul(p.c, make_float2(sr, si));
+}
+
+template <int M>
+__device__ __forceinline__ cf line_corr2_x(const FusedParams& p, const float* Ks, const long long grow, const int seg,
+                                           const int pidx) {
+    if (p.t == 8) return line_corr2_x_t<M, 8>(p, Ks, grow, seg, pidx);   // the paper's default
+    if (p.t == 4) return line_corr2_x_t<M, 4>(p, Ks, grow, seg, pidx);
+    return line_corr2_x_t<M, 0>(p, Ks, grow, seg, pidx);
 }
 
 template <class PL, int NWARP, int MODE>
