@@ -120,7 +120,7 @@ MBS_API int mbs_create(mbs_ctx** out, int ndim, const int64_t* shape, double pix
                const int32_t* boundary_width, const int32_t* n_subdomains, const uint8_t* periodic,
                int32_t n_correction, void* cuda_stream);
 
-/* 1 if a subdomain length M has an FFT plan in this build (2^a * 5^b sizes listed in DESIGN.md). */
+/* 1 if a subdomain length M has an FFT plan in this build: 2^a (8..1024), 5*2^a (40..640), 3*2^a (48..768). */
 MBS_API int mbs_fft_supported(int64_t M);
 
 /* Bytes of device workspace the context needs (B_diag, u, slab buffers, reduction scratch). */

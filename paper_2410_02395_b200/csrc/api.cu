@@ -292,7 +292,7 @@ extern "C" int mbs_create(mbs_ctx** out, int ndim, const int64_t* shape, double 
             else if (g.a[ax] > 0 && 2 * (int64_t)n_correction > M)
                 rc = fail(nullptr, MBS_ERR_INVALID_ARG, "2*n_correction = %d exceeds the subdomain length %lld of axis %d", 2 * n_correction, (long long)M, d);
             else if (!fft_lookup((int)M))
-                rc = fail(nullptr, MBS_ERR_UNSUPPORTED_SIZE, "no FFT plan for subdomain length %lld (axis %d); supported: 8..1024 powers of two and 40, 80, 160, 320, 640", (long long)M, d);
+                rc = fail(nullptr, MBS_ERR_UNSUPPORTED_SIZE, "no FFT plan for subdomain length %lld (axis %d); supported: 8..1024 powers of two, 40..640 (5*2^k) and 48..768 (3*2^k)", (long long)M, d);
             else c->fft[ax] = fft_lookup((int)M);
         }
     }

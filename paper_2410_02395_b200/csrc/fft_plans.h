@@ -1,4 +1,4 @@
-// fft_plans.h -- the subdomain lengths M this build has FFT plans for (2^a and 5*2^a), with the
+// fft_plans.h -- the subdomain lengths M this build has FFT plans for (2^a, 5*2^a and 3*2^a), with the
 // points per thread P, the pass radices and the lines per tile C of each.
 // BASELINE.json configs need 128 (cfg 1, 3), 256 (cfg 3, 5), 320 (cfg 4) and 512 (cfg 2, 5).
 #pragma once
@@ -21,8 +21,13 @@ template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        st
 template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int CS = 16, CC = 16; };
 template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 32, CC = 16; };
 template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<48>   { using type = Plan<48,   12, 12, 4>;        static constexpr int CS = 64, CC = 64; };
+template <> struct FftPlan<96>   { using type = Plan<96,   24, 12, 8>;        static constexpr int CS = 32, CC = 32; };
+template <> struct FftPlan<192>  { using type = Plan<192,  12, 12, 4, 4>;     static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<384>  { using type = Plan<384,  24, 12, 8, 4>;     static constexpr int CS = 16, CC = 16; };
+template <> struct FftPlan<768>  { using type = Plan<768,  24, 12, 8, 8>;     static constexpr int CS = 8, CC = 8;  };
 
 }  // namespace mbs
 
 #define MBS_FOR_EACH_FFT_SIZE(X) \
-    X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(40) X(80) X(160) X(320) X(640)
+    X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(40) X(80) X(160) X(320) X(640) X(48) X(96) X(192) X(384) X(768)

@@ -92,6 +92,10 @@ ITERATION_CASES = OPERATOR_CASES + [
     ((8, 8, 256), (1, 1, 2), (0, 0, 8), 8, (1, 1, 0)),       # periodic single-domain axes 0, 1: no slab rows
     ((48, 40, 64), (3, 1, 2), (4, 4, 4), 8, None),            # ragged tile tail: 48*40*2 lines is not a multiple of 16
     ((32, 32, 320), (2, 2, 1), (4, 4, 8), 8, None),
+    ((768,), (1,), (16,), 8, None),                            # 3 * 2^k line lengths
+    ((384,), (2,), (8,), 8, None),
+    ((96, 48), (1, 1), (4, 4), 8, None),
+    ((48, 48, 96), (1, 1, 1), (4, 4, 4), 4, None),
 ]
 
 
@@ -281,6 +285,19 @@ def test_argument_errors(B):
     assert e.value.status == B.MBS_ERR_STATE
     s.close()
     s2.close()
+
+
+def test_non_finite_residual_is_reported(B):
+    """A NaN in the source makes the residual non-finite: MBS_ERR_NUMERIC, not a silent run to max_iter (mbs.h)."""
+    w = workloads.config(3, shape=(32, 32, 64), boundary_width=(4, 4, 4))
+    s = B.Solver.from_workload(w)
+    s.set_potential(w.make_medium())
+    y = w.make_source()
+    y[3, 4, 5] = np.nan
+    with pytest.raises(B.MBSError) as e:
+        s.solve(y, tol=1e-3, max_iter=200)
+    assert e.value.status == B.MBS_ERR_NUMERIC
+    s.close()
 
 
 def test_periodic_undecomposed_matches_eq4(B, orc):
