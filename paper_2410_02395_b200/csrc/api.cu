@@ -792,9 +792,12 @@ static int ensure_history(mbs_ctx* c, int32_t max_iter) {
 
 // Enqueue `batch` iterations: as individual launches, or (graphs on, not profiling) as one replay of a CUDA graph
 // captured from the same launches.  The graph is rebuilt when the arrays, the batch or the kernel options change.
+static bool graphs_enabled(const mbs_ctx* c) {
+    return !c->profile && (c->use_graph == 1 || (c->use_graph < 0 && c->g.voxels <= (1LL << 25)));
+}
+
 static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_graph) {
-    const bool graph_on = allow_graph && !c->profile &&
-                          (c->use_graph == 1 || (c->use_graph < 0 && c->g.voxels <= (1LL << 25)));
+    const bool graph_on = allow_graph && graphs_enabled(c);
     if (!graph_on) {
         for (int i = 0; i < batch; ++i) MBS_TRY(run_iteration(c, y, x));
         return MBS_OK;
@@ -829,6 +832,12 @@ static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_g
     return MBS_OK;
 }
 
+// iterations enqueued between two looks at the device stop flag (and per CUDA-graph replay)
+static int poll_interval(const mbs_ctx* c) {
+    if (c->check_interval > 0) return c->check_interval;
+    return (int)std::max<long long>(1, std::min<long long>(64, (64LL << 20) / std::max<long long>(1, c->g.voxels)));
+}
+
 static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_iter, double* residual_history,
                         int32_t* n_iter) {
     if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
@@ -839,10 +848,7 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
     MBS_TRY(ensure_history(c, max_iter));
     MBS_TRY(begin_solve(c, y, tol, max_iter, 0.0));
 
-    int interval = c->check_interval;
-    if (interval <= 0) {
-        interval = (int)std::max<long long>(1, std::min<long long>(64, (64LL << 20) / std::max<long long>(1, c->g.voxels)));
-    }
+    const int interval = poll_interval(c);
     MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
     int enqueued = 0;
     int slot = 0;
@@ -853,7 +859,8 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
         // the first batch is enqueued launch by launch (it also warms the per-kernel attribute caches); later batches
         // replay a graph of a full interval: kernels past max_iter return at once on the device flag
         const bool first = (enqueued == 0);
-        const int batch = first ? std::min(interval, max_iter - enqueued) : (enqueued < max_iter ? interval : 0);
+        const int batch = (first || !graphs_enabled(c)) ? std::min(interval, max_iter - enqueued)
+                                                        : (enqueued < max_iter ? interval : 0);
         if (batch > 0 && !final_done) {
             MBS_TRY(enqueue_batch(c, y, x, batch, !first));
             enqueued += batch;
@@ -910,7 +917,18 @@ extern "C" int mbs_iterate(mbs_ctx* c, const void* y_device, void* x_device, int
     MBS_TRY(ensure_history(c, n_iter));
     MBS_TRY(begin_solve(c, (const cf*)y_device, -1.0, n_iter, nu));
     MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
-    for (int i = 0; i < n_iter; ++i) MBS_TRY(run_iteration(c, (const cf*)y_device, (cf*)x_device));
+    {
+        // first batch launch by launch, the rest as graph replays of a full interval (kernels past n_iter return at
+        // once on the device flag), exactly as mbs_solve enqueues them
+        const int interval = poll_interval(c);
+        int enqueued = 0;
+        while (enqueued < n_iter) {
+            const bool first = (enqueued == 0);
+            const int batch = (first || !graphs_enabled(c)) ? std::min(interval, n_iter - enqueued) : interval;
+            MBS_TRY(enqueue_batch(c, (const cf*)y_device, (cf*)x_device, batch, !first));
+            enqueued += batch;
+        }
+    }
     MBS_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));
     DevState fin{};
