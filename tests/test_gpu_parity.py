@@ -316,3 +316,45 @@ def test_periodic_undecomposed_matches_eq4(B, orc):
     assert rc == B.MBS_OK and abs(len(hist) - len(h_ref)) <= 1
     assert rel(x.cpu().numpy(), x_ref) <= FIELD_TOL
     s.close()
+
+
+def test_full_size_properties_cfg5(B):
+    """BASELINE.json config 5 at full size (1024^3, 4x2x2 subdomains) in the launch configuration bench.py times.
+    A converged oracle run is out of reach there, so this checks properties that hold at any
+    size: eps_0 = 1 and monotone decrease, the fused iteration against the one-kernel-per-step operators
+    of the same library (both are oracle-checked at small sizes), and (L+I)^-1 (L+I) = I on a random field."""
+    import torch
+    if torch.cuda.mem_get_info()[0] < 90 * 2 ** 30:
+        pytest.skip("needs about 80 GiB of free device memory")
+    w = workloads.config(5)
+    n, y = w.make_medium(), w.make_source()
+    s = B.Solver.from_workload(w)
+    s.set_potential(torch.from_numpy(n).cuda())
+    del n
+    yd = torch.from_numpy(y).cuda()
+    xd = torch.zeros(w.shape, dtype=torch.complex64, device="cuda")
+    hist = s.iterate(yd, xd, 12)
+    nu = s.info()["norm_rhs"]
+    assert hist[0] == pytest.approx(1.0, abs=1e-5)
+    assert np.all(np.diff(hist) < 0.0)
+    # residual of the current iterate from the unfused operators: r = B (x - (L+I)^-1 (B x + y_vec))
+    c = s.info()["c"]
+    t = s.apply_operator(B.MBS_OP_B, xd)
+    t.add_(yd, alpha=-c)                                   # y_vec = -c y (P:45)
+    t = s.apply_operator(B.MBS_OP_PROPAGATOR, t, out=t)
+    torch.sub(xd, t, out=t)
+    r = s.apply_operator(B.MBS_OP_B, t, out=t)
+    eps_unfused = float(torch.linalg.vector_norm(r)) / nu
+    eps_fused = s.iterate(yd, xd.clone(), 1, nu=nu)[0]
+    assert eps_fused == pytest.approx(eps_unfused, rel=2e-5)
+    # (L+I)^-1 [A u + B u] = u  (A = (L+I) - B, P:68)
+    del r, t
+    g = torch.Generator(device="cuda").manual_seed(5)
+    u = torch.randn(w.shape + (2,), generator=g, device="cuda", dtype=torch.float32)
+    u = torch.view_as_complex(u)
+    v = s.apply_operator(B.MBS_OP_A, u)
+    v.add_(s.apply_operator(B.MBS_OP_B, u))
+    v = s.apply_operator(B.MBS_OP_PROPAGATOR, v, out=v)
+    err = float(torch.linalg.vector_norm(v - u) / torch.linalg.vector_norm(u))
+    assert err <= OP_TOL, err
+    s.close()
