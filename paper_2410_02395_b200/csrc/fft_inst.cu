@@ -71,18 +71,6 @@ __global__ void __launch_bounds__(NTC) k_fused(const FusedParams p, const cf* __
     fused_contig_body<PL, CC, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
 }
 
-// staged variant of the first / last sweep (bulk-async copies of x and B_diag a tile ahead)
-constexpr bool staged_ok() { return PL::T <= 32 && 32 % PL::T == 0 && (PL::T * CC) % 32 == 0; }
-
-template <int MODE>
-__global__ void __launch_bounds__(NTC) k_fused_staged(const FusedParams p, const cf* __restrict__ tw, const int* __restrict__ done) {
-    extern __shared__ __align__(128) unsigned char smem_raw[];
-    __shared__ double red[32];
-    if (done && *done) return;
-    if constexpr (staged_ok() && (MODE == FUSED_S1 || MODE == FUSED_S5))
-        fused_staged_body<PL, CC, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
-}
-
 // warp-line variant of the first / last sweep (line_kernels.cuh): 8 warps per CTA, each warp owns whole lines
 constexpr bool line_ok() { return PL::T <= 32 && 32 % PL::T == 0; }
 constexpr int LINE_WARPS = 8;
@@ -174,16 +162,10 @@ cudaError_t run_contig(const cf* src, cf* dst, const ContigGeom& g, const Symbol
 }
 
 template <int MODE>
-constexpr bool use_staged(int t) {
-    return staged_ok() && MODE != FUSED_1D && fused_staged_smem_bytes<PL, CC>(t) <= 227 * 1024;
-}
-
-template <int MODE>
 cudaError_t fused_grid(int t, long long n_tiles, int num_sms, int* nb_out, size_t* smem_out) {
-    const bool staged = use_staged<MODE>(t);
-    const size_t smem = staged ? fused_staged_smem_bytes<PL, CC>(t) : sizeof(cf) * fused_smem_elems<PL, CC>(t);
+    const size_t smem = sizeof(cf) * fused_smem_elems<PL, CC>(t);
     int bps = 1;
-    cudaError_t e = staged ? prepare(k_fused_staged<MODE>, NTC, smem, &bps) : prepare(k_fused<MODE>, NTC, smem, &bps);
+    cudaError_t e = prepare(k_fused<MODE>, NTC, smem, &bps);
     if (e != cudaSuccess) return e;
     long long nb = (long long)num_sms * bps;
     if (nb > n_tiles) nb = n_tiles;
@@ -200,8 +182,7 @@ cudaError_t run_fused(const FusedParams& p, const cf* tw, const int* done, int n
     size_t smem = 0;
     cudaError_t e = fused_grid<MODE>(p.t, p.n_tiles, num_sms, &nb, &smem);
     if (e != cudaSuccess) return e;
-    if (use_staged<MODE>(p.t)) k_fused_staged<MODE><<<(unsigned)nb, NTC, smem, st>>>(p, tw, done);
-    else k_fused<MODE><<<(unsigned)nb, NTC, smem, st>>>(p, tw, done);
+    k_fused<MODE><<<(unsigned)nb, NTC, smem, st>>>(p, tw, done);
     return cudaGetLastError();
 }
 

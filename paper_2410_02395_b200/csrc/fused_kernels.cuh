@@ -18,7 +18,6 @@
 //      the fix-up kernels (kernels.cu) then apply corr_0(d), corr_1(d) there.
 #pragma once
 #include "fft_kernels.cuh"
-#include "fft_tma.cuh"
 #include "reduce.cuh"
 
 namespace mbs {
@@ -82,7 +81,7 @@ template <int M, bool SLAB>
 __device__ __forceinline__ void fused_pro_line(const FusedParams& p, const cf* xl, const cf* bl, const long long gl, cf* trow,
                                                const cf* cel, const int lane, const bool has_y, const long long o0,
                                                const long long o1) {
-    // xl, bl: this line of x and B_diag (global memory, or the shared-memory stage of the staged kernel)
+    // xl, bl: this line of x and B_diag
     constexpr int EP2 = (M + 63) / 64;
     const int t = p.t;
     const cf* yl = p.y + gl;
@@ -301,212 +300,6 @@ __device__ __forceinline__ void fused_contig_body(const FusedParams& p, const cf
         }
     }
     if constexpr (MODE != FUSED_S1) {
-        const double bs = block_sum((double)acc, red);
-        grid_reduce_finish(bs, p.partials, p.slot0, p.n_total, p.finish, p.reduce_mode, p.state, p.hist, red);
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// Staged variant of FUSED_S1 / FUSED_S5 (persistent CTA, one bulk-async copy per array per tile).
-// A tile's rows are one contiguous chunk of C*M voxels, so x and B_diag of a tile arrive with two
-// `cp.async.bulk` copies that signal an mbarrier; they are issued a tile ahead and land in the stages A
-// (x) and B (B_diag) while the butterflies of the current tile run, so no phase waits on HBM latency:
-//   S1:  [wait A,B] prologue(A,B -> tile) | issue A,B of tile i+1 | FFT | store u
-//   S5:  FFT(tile = u'_i) | load u'_{i+1} into registers | [wait A,B] epilogue(tile,A,B) |
-//        issue A,B of tile i+1 | registers -> tile
-// ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ void bulk_load(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-
-template <class PL, int C>
-constexpr size_t fused_staged_smem_bytes(int t) {
-    return sizeof(cf) * (size_t)(2 * C * PL::M + fused_smem_elems<PL, C>(t)) + 16;
-}
-
-template <class PL, int C, int MODE>
-__device__ __forceinline__ void fused_staged_body(const FusedParams& p, const cf* __restrict__ tw_global, cf* smem, double* red) {
-    static_assert(MODE == FUSED_S1 || MODE == FUSED_S5, "staged variant: first or last sweep");
-    constexpr int M = PL::M, P = PL::P, T = PL::T, NT = T * C, LS = M + 1;
-    static_assert(T <= 32 && 32 % T == 0 && M % 2 == 0, "one warp holds whole lines");
-    constexpr int NW = NT / 32;
-    constexpr int LPW = C / NW;                       // lines per warp
-    constexpr int EP2 = (M + 63) / 64;
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int t = p.t, t2 = 2 * p.t;
-    cf* sA = smem;                                    // stage: x of the tile      [C][M]
-    cf* sB = sA + C * M;                              // stage: B_diag of the tile [C][M]
-    cf* tw = sB + C * M;
-    cf* tile = tw + M;
-    cf* ed = tile + C * LS;
-    cf* ce = ed + C * t2;
-    float* Ks = reinterpret_cast<float*>(ce + C * t2);
-    long long* loff = reinterpret_cast<long long*>(Ks + ((t * t + 1) / 2) * 2);
-    int* lflag = reinterpret_cast<int*>(loff + 2 * C);
-    unsigned long long* bar = reinterpret_cast<unsigned long long*>(lflag + 2 * ((C + 1) / 2));
-    for (int i = tid; i < M; i += NT) tw[i] = tw_global[i];
-    if (p.a2) for (int i = tid; i < t * t; i += NT) Ks[i] = p.Kh[i];
-    if (tid == 0) {
-        mbar_init(bar, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-        fence_async_smem();
-    }
-    __syncthreads();
-    const int c_ = tid % C, jt = tid / C;
-    const unsigned n_lines = (unsigned)p.n_lines, n_tiles = (unsigned)p.n_tiles;
-    auto valid_lines = [&](unsigned tix) { return (int)((n_lines - tix * C) < (unsigned)C ? (n_lines - tix * C) : (unsigned)C); };
-    auto issue = [&](unsigned tix) {                  // thread 0: x and B_diag of tile tix -> stages
-        const long long g0 = (long long)tix * C * M;
-        const unsigned bytes = (unsigned)valid_lines(tix) * M * (unsigned)sizeof(cf);
-        mbar_expect_tx(bar, 2 * bytes);
-        bulk_load(sA, p.x + g0, bytes, bar);
-        bulk_load(sB, p.bdiag + g0, bytes, bar);
-    };
-    cf2 ureg[LPW][EP2];                               // S5: u' of the next tile, in flight during the epilogue
-    auto load_u = [&](unsigned tix) {
-        const long long g0 = (long long)tix * C * M;
-        const int nv = valid_lines(tix);
-#pragma unroll
-        for (int j = 0; j < LPW; ++j) {
-            const int line = warp + j * NW;
-#pragma unroll
-            for (int k = 0; k < EP2; ++k) {
-                const int q = 2 * lane + 64 * k;
-                if (line < nv && (M % 64 == 0 || q < M)) ureg[j][k] = ld2(p.u + g0 + (long long)line * M + q);
-            }
-        }
-    };
-    auto put_u = [&](unsigned tix) {
-        const int nv = valid_lines(tix);
-#pragma unroll
-        for (int j = 0; j < LPW; ++j) {
-            const int line = warp + j * NW;
-#pragma unroll
-            for (int k = 0; k < EP2; ++k) {
-                const int q = 2 * lane + 64 * k;
-                if (line < nv && (M % 64 == 0 || q < M)) {
-                    tile[line * LS + q] = ureg[j][k].a;
-                    tile[line * LS + q + 1] = ureg[j][k].b;
-                }
-            }
-        }
-    };
-    unsigned tix = blockIdx.x;
-    if (tix < n_tiles) {
-        if (tid == 0) issue(tix);
-        if constexpr (MODE == FUSED_S5) {
-            load_u(tix);
-            put_u(tix);
-        }
-    }
-    float acc = 0.f;
-    unsigned parity = 0;
-    for (; tix < n_tiles; tix += gridDim.x, parity ^= 1u) {
-        const unsigned line0 = tix * C;
-        const int nvalid = valid_lines(tix);
-        const long long g0 = (long long)line0 * M;
-        const bool more = tix + gridDim.x < n_tiles;
-        if (tid < nvalid) fused_line_info<M>(p, line0 + tid, loff + 2 * tid, lflag + tid);
-        if constexpr (MODE == FUSED_S1) {
-            mbar_wait(bar, parity);
-            if (p.a2) {
-                for (int o = tid; o < nvalid * t2; o += NT) {
-                    const int line = o / t2, e = o - line * t2;
-                    ed[o] = sA[line * M + (e < t ? e : M - t2 + e)];
-                }
-                __syncthreads();
-                fused_corr2<C>(ed, ce, Ks, t, p.S2, p.per2, p.c, nvalid, tid, NT);
-            }
-            __syncthreads();
-#pragma unroll
-            for (int j = 0; j < LPW; ++j) {
-                const int line = warp + j * NW;
-                if (line < nvalid) {
-                    const long long gl = g0 + (long long)line * M;
-                    const long long o0 = loff[2 * line], o1 = loff[2 * line + 1];
-                    const bool has_y = lflag[line] != 0;
-                    if (o0 >= 0 || o1 >= 0)
-                        fused_pro_line<M, true>(p, sA + line * M, sB + line * M, gl, tile + line * LS, ce + line * t2, lane, has_y, o0, o1);
-                    else
-                        fused_pro_line<M, false>(p, sA + line * M, sB + line * M, gl, tile + line * LS, ce + line * t2, lane, has_y, o0, o1);
-                }
-            }
-            __syncthreads();                          // stages consumed, tile complete
-            if (tid == 0 && more) issue(tix + gridDim.x);
-        } else {
-            __syncthreads();                          // u' of this tile is in place
-        }
-        // ---- FFT along the line ----
-        cf v[P];
-        static_for<0, P>([&](auto mc) {
-            constexpr int m = decltype(mc)::value;
-            v[m] = tile[c_ * LS + jt + m * T];
-        });
-        if constexpr (PL::NPASS > 1) __syncthreads();
-        if constexpr (MODE == FUSED_S5) {
-            static_for<0, P>([&](auto mc) { v[decltype(mc)::value] = cswap(v[decltype(mc)::value]); });
-        }
-#ifndef MBS_DBG_NOFFT
-        fft_line_forward<PL, 1, LS>(v, tile, c_, jt, tw);
-#endif
-        if constexpr (MODE == FUSED_S5) {
-            static_for<0, P>([&](auto mc) { v[decltype(mc)::value] = cswap(v[decltype(mc)::value]); });
-        }
-        static_for<0, P>([&](auto mc) {
-            constexpr int m = decltype(mc)::value;
-            tile[c_ * LS + jt + m * T] = v[m];
-        });
-        __syncthreads();
-        if constexpr (MODE == FUSED_S1) {
-#pragma unroll
-            for (int j = 0; j < LPW; ++j) {
-                const int line = warp + j * NW;
-                if (line < nvalid) {
-                    cf* ul = p.u + g0 + (long long)line * M;
-                    const cf* trow = tile + line * LS;
-#pragma unroll
-                    for (int k = 0; k < EP2; ++k) {
-                        const int q = 2 * lane + 64 * k;
-                        if (M % 64 == 0 || q < M) st2(ul + q, trow[q], trow[q + 1]);
-                    }
-                }
-            }
-            __syncthreads();                          // tile free for the next prologue
-        } else {
-            if (more) load_u(tix + gridDim.x);        // in flight during the epilogue
-            mbar_wait(bar, parity);
-            if (p.a2) {
-                for (int o = tid; o < nvalid * t2; o += NT) {
-                    const int line = o / t2, e = o - line * t2;
-                    const int q = (e < t ? e : M - t2 + e);
-                    ed[o] = csub(sA[line * M + q], tile[line * LS + q]);
-                }
-                __syncthreads();
-                fused_corr2<C>(ed, ce, Ks, t, p.S2, p.per2, p.c, nvalid, tid, NT);
-                __syncthreads();
-            }
-#pragma unroll
-            for (int j = 0; j < LPW; ++j) {
-                const int line = warp + j * NW;
-                if (line < nvalid) {
-                    const long long gl = g0 + (long long)line * M;
-                    const long long o0 = loff[2 * line], o1 = loff[2 * line + 1];
-                    if (o0 >= 0 || o1 >= 0)
-                        fused_epi_line<M, true>(p, sA + line * M, sB + line * M, gl, tile + line * LS, ce + line * t2, lane, o0, o1);
-                    else
-                        acc += fused_epi_line<M, false>(p, sA + line * M, sB + line * M, gl, tile + line * LS, ce + line * t2, lane, o0, o1);
-                }
-            }
-            __syncthreads();                          // tile and stages consumed
-            if (more) {
-                if (tid == 0) issue(tix + gridDim.x);
-                put_u(tix + gridDim.x);
-            }
-        }
-    }
-    if constexpr (MODE == FUSED_S5) {
         const double bs = block_sum((double)acc, red);
         grid_reduce_finish(bs, p.partials, p.slot0, p.n_total, p.finish, p.reduce_mode, p.state, p.hist, red);
     }
