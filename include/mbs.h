@@ -152,7 +152,9 @@ MBS_API int mbs_apply_operator(mbs_ctx* ctx, int which, const void* in_device, v
  *  residual_history  host, capacity max_iter (may be NULL): history[n] = eps_n, the relative
  *      residual ||Gamma^-1(y - A x^(n))|| / ||Gamma^-1 y|| of the iterate BEFORE update n.
  *  n_iter  host, out: number of updates applied.
- * Returns MBS_OK (converged), MBS_ERR_NOT_CONVERGED, MBS_ERR_NUMERIC, or a CUDA/state error.
+ * Returns MBS_OK (converged), MBS_ERR_NOT_CONVERGED, MBS_ERR_NUMERIC (NaN/Inf in the source, the medium or the
+ * residual), MBS_ERR_INVALID_ARG (y identically zero: the relative residual of P:130 is undefined), or a
+ * CUDA/state error.
  */
 MBS_API int mbs_solve(mbs_ctx* ctx, const void* y_device, void* x_device, double tol, int32_t max_iter,
               double* residual_history, int32_t* n_iter);

@@ -776,6 +776,15 @@ static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, do
         MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
     }
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));   // state_pinned[0] is reused by the poll loop
+    if (!(nu > 0)) {
+        // the relative residual of P:130 divides by ||Gamma^-1 y_vec||: a zero (or non-finite) source has none
+        DevState st{};
+        MBS_CUDA(c, cudaMemcpy(&st, c->state, sizeof(DevState), cudaMemcpyDeviceToHost));
+        if (!(st.nu2 > 0) || !std::isfinite(st.nu2))
+            return fail(c, st.nu2 == 0 ? MBS_ERR_INVALID_ARG : MBS_ERR_NUMERIC,
+                        st.nu2 == 0 ? "the source y is identically zero: ||Gamma^-1 y|| = 0 and the relative residual is undefined"
+                                    : "non-finite ||Gamma^-1 y||: the source or the medium holds NaN/Inf");
+    }
     return MBS_OK;
 }
 

@@ -132,9 +132,20 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
                 issue_load(i + NSTAGE - 1);
             }
         }
-        mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
         int c0, c1, c2, ii0;
         coords(i, c0, c1, c2, ii0);
+        // |p|^2 of the other axes for this thread's line: requested before the wait so its latency is covered
+        float wline = 0.f;
+        if constexpr (MODE == FFT_MID) {
+            const int ii = ii0 + c;
+            if (sp.wtab) {
+                wline = ii < g.inner ? sp.wtab[ii] : 0.f;
+            } else {
+                if (sp.tabA) wline += sp.tabA[(ii / sp.Nb) % sp.Ma];
+                if (sp.tabB) wline += sp.tabB[(ii % sp.Nb) % sp.Mb];
+            }
+        }
+        mbar_wait(&full[s], (unsigned)((i / NSTAGE) & 1));
         cf v[P];
         static_for<0, P>([&](auto mc) {
             constexpr int m = decltype(mc)::value;
@@ -146,14 +157,6 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
         }
         fft_line_forward<PL, C, 1>(v, tile, c, jt, tw);
         if constexpr (MODE == FFT_MID) {
-            const int ii = ii0 + c;
-            float wline = 0.f;
-            if (sp.wtab) {
-                wline = ii < g.inner ? sp.wtab[ii] : 0.f;       // |p|^2 of the other axes, one value per line
-            } else {
-                if (sp.tabA) wline += sp.tabA[(ii / sp.Nb) % sp.Ma];
-                if (sp.tabB) wline += sp.tabB[(ii % sp.Nb) % sp.Mb];
-            }
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
                 v[m] = cswap(apply_symbol(v[m], p2a[m] + wline, sp));

@@ -297,6 +297,29 @@ def test_non_finite_residual_is_reported(B):
     with pytest.raises(B.MBSError) as e:
         s.solve(y, tol=1e-3, max_iter=200)
     assert e.value.status == B.MBS_ERR_NUMERIC
+    # a NaN that appears later (in the start vector) is caught by the residual check of the loop
+    y = w.make_source()
+    x0 = np.zeros(w.shape, dtype=np.complex64)
+    x0[1, 2, 3] = np.nan
+    with pytest.raises(B.MBSError) as e:
+        s.solve(y, x0=x0, tol=1e-3, max_iter=200)
+    assert e.value.status == B.MBS_ERR_NUMERIC
+    s.close()
+
+
+def test_degenerate_inputs(B):
+    """Zero source: no relative residual -> MBS_ERR_INVALID_ARG.  Homogeneous periodic medium without any
+    correction: V = 0, Eq. (4) has no scale -> MBS_ERR_INVALID_ARG at set_potential."""
+    s = B.Solver((64, 64), 0.25, 1.0, (4, 4), (2, 1), n_correction=8)
+    s.set_potential(workloads.random_medium((64, 64), 3))
+    with pytest.raises(B.MBSError) as e:
+        s.solve(np.zeros((64, 64), dtype=np.complex64), tol=1e-3, max_iter=10)
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
+    s.close()
+    s = B.Solver((64,), 0.25, 1.0, (0,), (1,), periodic=(1,), n_correction=0)
+    with pytest.raises(B.MBSError) as e:
+        s.set_potential(np.full(64, 1.3 + 0.0j, dtype=np.complex64))
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
     s.close()
 
 
