@@ -70,6 +70,9 @@ enum mbs_option {
                                    shared-memory stage ring; 0: threads load/store the tiles themselves        */
     MBS_OPT_LINE = 5,           /* 1 (default): first / last sweep as warp-line kernels (each warp owns whole lines of
                                    the contiguous axis, no block barriers); 0: tile kernels with in-CTA edge terms  */
+    MBS_OPT_MERGE = 6,          /* 1: the last sweep also runs the next iteration's first sweep on every row outside the
+                                   axis-0/1 slabs (saves the re-read of x and B_diag, 96 B ledger); needs MBS_OPT_LINE.
+                                   Default 0: with 128 registers per thread it is latency-bound and measured slower  */
     MBS_OPT_PROFILE = 3         /* 1: bracket every kernel launch with CUDA events on the context's stream and
                                    accumulate per-kernel device time (mbs_get_kernel_stats); disables graphs   */
 };

@@ -89,6 +89,36 @@ __device__ __forceinline__ cf line_corr2_x(const FusedParams& p, const float* Ks
     return line_corr2_x_t<M, 0>(p, Ks, grow, seg, pidx);
 }
 
+__device__ __forceinline__ int line_edge_index(int q, int M, int t) {   // q in [0, S*2t) -> index along the axis
+    const int s = q / (2 * t), e = q - s * 2 * t;
+    return s * M + (e < t ? e : M - 2 * t + e);
+}
+
+// k-th row (in the enumeration of k_fixup: set A = {i0 edge of axis 0} x all i1, then set B = {i0 not an edge of
+// axis 0} x {i1 edge of axis 1}) -> row index i0 * N1 + i1
+__device__ __forceinline__ unsigned line_slab_row(const FusedParams& p, unsigned rid) {
+    const int t = p.t;
+    const unsigned nE0 = p.e0 ? (unsigned)(p.S0 * 2 * t) : 0u, nE1 = p.e1 ? (unsigned)(p.S1 * 2 * t) : 0u;
+    const unsigned rowsA = nE0 * (unsigned)p.N1;
+    int i0, i1;
+    if (rid < rowsA) {
+        const unsigned q0 = rid / (unsigned)p.N1;
+        i1 = (int)(rid - q0 * (unsigned)p.N1);
+        i0 = line_edge_index((int)q0, p.M0, t);
+    } else {
+        const unsigned rb = rid - rowsA;
+        const unsigned k0 = rb / nE1;
+        i1 = line_edge_index((int)(rb - k0 * nE1), p.M1, t);
+        if (p.e0) {
+            const int w = p.M0 - 2 * t, s = (int)k0 / w;
+            i0 = s * p.M0 + t + ((int)k0 - s * w);
+        } else {
+            i0 = (int)k0;
+        }
+    }
+    return (unsigned)i0 * (unsigned)p.N1 + (unsigned)i1;
+}
+
 template <class PL, int NWARP, int MODE>
 __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __restrict__ tw_global, cf* smem, double* red) {
     constexpr int M = PL::M, P = PL::P, T = PL::T, NT = NWARP * 32;
@@ -108,10 +138,14 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
     const unsigned n_units = (n_lines + LW - 1) / LW;
     float acc = 0.f;
     for (unsigned unit = blockIdx.x * NWARP + warp; unit < n_units; unit += gridDim.x * NWARP) {
-        const unsigned line = unit * LW + lsub;
+        unsigned line = unit * LW + lsub;
         const bool valid = line < n_lines;
-        const unsigned row = line / (unsigned)p.S2;
+        unsigned row = line / (unsigned)p.S2;
         const int seg = (int)(line - row * (unsigned)p.S2);
+        if (MODE == LINE_S1 && p.slab_rows_only) {    // `line` counted slab-row lines: map to the real row
+            row = valid ? line_slab_row(p, row) : 0u;
+            line = row * (unsigned)p.S2 + (unsigned)seg;
+        }
         const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
         long long o0 = -1, o1 = -1;                   // compact row offsets of the axis-0 / axis-1 slabs
         if (valid && p.e0) {

@@ -141,7 +141,7 @@ cudaError_t launch_setup(const GridDesc& g, const SetupParams& p, int pass, doub
 
 // fused first / last sweep along the contiguous axis (fused_kernels.cuh)
 enum FusedMode { FUSED_S1 = 0, FUSED_S5 = 1, FUSED_1D = 2 };
-enum LineMode { LINE_S1 = 0, LINE_S5 = 1 };   // warp-line variant (line_kernels.cuh)
+enum LineMode { LINE_S1 = 0, LINE_S5 = 1, LINE_S51 = 2 };   // warp-line variant (line_kernels.cuh)
 
 struct FusedParams {
     cf* x;               // iterate: read by S1; read and updated in place by S5 / 1D
@@ -150,7 +150,9 @@ struct FusedParams {
     const unsigned char* ymask;   // per grid row: 0 = the row of y is all zero (skip its load); nullptr = unknown
     cf ysc;              // y_vec = ysc * y = -c y
     cf* u;               // S1: output; S5: input u' lines, output r_part on slab rows
-    int N1, N2;          // extents of axes 1 and 2 (N2 = S2 * M)
+    int N0, N1, N2;      // grid extents (N2 = S2 * M)
+    int S0;              // subdomains along axis 0
+    int slab_rows_only;  // warp-line sweep 1: visit only the rows that lie in a slab of axis 0 or 1 (n_lines counts those)
     int S2, a2, per2;    // subdomains, a_d and periodic flag of the last axis
     int t;               // correction points
     int e0, e1;          // 1 if axis 0 / 1 has edge corrections
@@ -188,6 +190,10 @@ struct FftEntry {
     // warp-line variant of the first / last sweep (line_kernels.cuh); nullptr when a line does not fit in a warp
     cudaError_t (*line)(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st);
     int (*line_blocks)(int mode, int t, long long n_lines, int num_sms);
+    // last sweep merged with the next iteration's first sweep (line_merged.cuh); merged_blocks = grid size, 0 if the
+    // number of subdomains along the last axis does not map onto whole warps of one CTA
+    cudaError_t (*merged)(const FusedParams& p, const cf* tw, const int* done, int num_sms, cudaStream_t st);
+    int (*merged_blocks)(int S2, int t, long long n_lines, int num_sms);
 };
 const FftEntry* fft_lookup(int M);
 

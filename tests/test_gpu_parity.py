@@ -99,9 +99,9 @@ ITERATION_CASES = OPERATOR_CASES + [
 ]
 
 
-@pytest.mark.parametrize("fused,tma,line", [(1, 1, 1), (1, 1, 0), (0, 1, 1), (1, 0, 0)])
+@pytest.mark.parametrize("fused,tma,line,merge", [(1, 1, 1, 1), (1, 1, 1, 0), (1, 1, 0, 0), (0, 1, 1, 0), (1, 0, 0, 0)])
 @pytest.mark.parametrize("shape,S,W,t,periodic", ITERATION_CASES)
-def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line):
+def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line, merge):
     """A few updates of Eq. (6) from a random start with a dense random source, fused sweeps and
     one-kernel-per-step path, against the oracle's iterates: every step of SURVEY 8(a) on every geometry."""
     import torch
@@ -109,6 +109,7 @@ def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line):
     s.set_option(B.MBS_OPT_FUSED, fused)
     s.set_option(B.MBS_OPT_TMA, tma)
     s.set_option(B.MBS_OPT_LINE, line)
+    s.set_option(B.MBS_OPT_MERGE, merge)
     y = workloads.random_field(shape, 21)
     x0 = workloads.random_field(shape, 22)
     n_it = 6
