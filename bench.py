@@ -101,7 +101,7 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_sample(cfg, n_iter, budget_s=25.0):
+def oracle_sample(cfg, n_iter, budget_s=25.0, warmup=1):
     """Time the CPU oracle (oracle/mbs_oracle.py, as it stands) on a bounded sample of config `cfg`: the same
     generator and subdomain counts at a reduced grid, `n_iter` iterations of Eq. (6).  Returns a dict."""
     from paper_2410_02395_b200 import workloads
@@ -125,13 +125,18 @@ def oracle_sample(cfg, n_iter, budget_s=25.0):
         o.solve(y, tol=0.0, max_iter=n_iter, callback=cb)
     except StopIteration:
         pass
-    # the first callback interval also holds the nu pre-pass: drop it when there are more
-    steady = times[1:] if len(times) > 1 else times
+    # the first callback interval also holds the nu pre-pass: the warm-up iterations are dropped when there are more
+    steady = times[warmup:] if len(times) > warmup else times[-1:]
     per_it = float(np.mean(steady))
     return {"value": w.voxels / per_it / 1e9, "unit": UNIT, "cores": mbs_oracle._workers(), "kind": "oracle",
             "sample": "cfg%d generator at %s with %s subdomains, %d oracle iterations (numpy complex128, scipy.fft)"
                       % (cfg, "x".join(map(str, shape)), "x".join(map(str, w.n_subdomains)), len(steady)),
             "ms_per_step": per_it * 1e3, "voxels": w.voxels}
+
+
+def _workloads():
+    from paper_2410_02395_b200 import workloads
+    return workloads
 
 
 def run_reference(args):
@@ -141,11 +146,11 @@ def run_reference(args):
         return
     K = args.steps if args.steps is not None else 5
     W = args.warmup if args.warmup is not None else 1
-    r = oracle_sample(args.config, K + W, budget_s=120.0)
+    r = oracle_sample(args.config, K + W, budget_s=120.0, warmup=W)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": K,
             "warmup": W, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "c128", "data": "synthetic",
-            "config": {"workload": workload_name(__import__("paper_2410_02395_b200.workloads", fromlist=["config"]).config(args.config)),
+            "config": {"workload": workload_name(_workloads().config(args.config)),
                        "sample": r["sample"]},
             "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
