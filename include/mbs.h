@@ -18,6 +18,8 @@
  *    (unless mbs_set_workspace is used) its workspace.
  *  - Every call returns an int status (MBS_OK = 0).  No exceptions cross the boundary, there is
  *    no global state, and one context must be used from one thread at a time.
+ *  - A context belongs to the CUDA device that is current when mbs_create is called; every later call on it must be
+ *    made with the same current device.
  *  - All device work is enqueued on the stream given to mbs_create.  mbs_apply_operator and
  *    mbs_set_potential are asynchronous with respect to the host unless stated; mbs_solve*
  *    return after the stop decision has been observed.

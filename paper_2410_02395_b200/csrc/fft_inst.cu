@@ -103,16 +103,18 @@ __global__ void __launch_bounds__(LINE_WARPS * 32, 2) k_line_merged(const FusedP
 // (The attribute must be raised again when a later launch needs more than the size it was set to.)
 template <class K>
 cudaError_t prepare(K kernel, int nthreads, size_t smem, int* blocks_per_sm) {
-    struct Entry { const void* fn; size_t smem; size_t attr; int bps; };
-    static thread_local Entry cache[16];
+    struct Entry { const void* fn; int dev; size_t smem; size_t attr; int bps; };
+    static thread_local Entry cache[32];
     static thread_local int n_cached = 0;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);              // function attributes are per device
+    if (e != cudaSuccess) return e;
     size_t attr = 0;
     for (int i = 0; i < n_cached; ++i) {
-        if (cache[i].fn != (const void*)kernel) continue;
+        if (cache[i].fn != (const void*)kernel || cache[i].dev != dev) continue;
         if (cache[i].smem == smem) { *blocks_per_sm = cache[i].bps; return cudaSuccess; }
         if (cache[i].attr > attr) attr = cache[i].attr;
     }
-    cudaError_t e;
     if (smem > attr) {
         e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
@@ -122,7 +124,7 @@ cudaError_t prepare(K kernel, int nthreads, size_t smem, int* blocks_per_sm) {
     e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, nthreads, smem);
     if (e != cudaSuccess) return e;
     if (bps < 1) bps = 1;
-    if (n_cached < 16) cache[n_cached++] = Entry{(const void*)kernel, smem, attr, bps};
+    if (n_cached < 32) cache[n_cached++] = Entry{(const void*)kernel, dev, smem, attr, bps};
     *blocks_per_sm = bps;
     return cudaSuccess;
 }
