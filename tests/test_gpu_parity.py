@@ -382,3 +382,34 @@ def test_full_size_properties_cfg5(B):
     err = float(torch.linalg.vector_norm(v - u) / torch.linalg.vector_norm(u))
     assert err <= OP_TOL, err
     s.close()
+
+
+MID_SIZE_CASES = [
+    ("cfg4_160", lambda: workloads.config(4, shape=(160, 160, 160), boundary_width=(12, 12, 12))),
+    ("cfg5_256", lambda: workloads.config(5, shape=(256, 256, 256), boundary_width=(16, 16, 16))),
+]
+
+
+@pytest.mark.parametrize("name,make", MID_SIZE_CASES)
+def test_operators_and_first_residuals_mid_size(B, orc, name, make):
+    """Parity plan of SURVEY 8(d) for configs 4-5 at the largest size the oracle handles in about a minute (same
+    generators and subdomain counts): (i) per-operator parity on a seeded random vector, (ii) the first 10 residuals."""
+    import torch
+    w = make()
+    n, y = w.make_medium(), w.make_source()
+    o = orc.from_workload(w, n)
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    u = workloads.random_field(w.shape, 31)
+    u128 = u.astype(np.complex128)
+    for which, ref in ((B.MBS_OP_B, o.apply_B(u128)), (B.MBS_OP_PROPAGATOR, o.propagate(u128)),
+                       (B.MBS_OP_PRECOND_A, o.apply_precond_A(u128))):
+        got = s.apply_operator(which, u).cpu().numpy()
+        assert rel(got, ref) <= OP_TOL, (which, rel(got, ref))
+    x_ref, h_ref = o.solve(y, tol=0.0, max_iter=10)
+    yd = torch.from_numpy(y).cuda()
+    xd = torch.zeros(w.shape, dtype=torch.complex64, device="cuda")
+    hist = s.iterate(yd, xd, 10)
+    assert np.allclose(hist, h_ref, rtol=1e-4), (hist, h_ref)
+    assert rel(xd.cpu().numpy(), x_ref) <= OP_TOL
+    s.close()
