@@ -565,7 +565,8 @@ static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, b
     for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
     for (int d = 0; d < ax; ++d) outer *= g.N[d];
     sg.stride = inner; sg.outer_stride = (long long)g.N[ax] * inner; sg.n_outer = (int)outer; sg.n_seg = g.S[ax];
-    sg.inner = (int)inner; sg.tiles_inner = (int)((inner + e->CS - 1) / e->CS);
+    const int cs = (mode == FFT_MID) ? e->CSM : e->CS;
+    sg.inner = (int)inner; sg.tiles_inner = (int)((inner + cs - 1) / cs);
     sg.n_tiles = outer * g.S[ax] * sg.tiles_inner;
     SymbolParams s2 = make_symbol(c, inverse);
     s2.tab_axis = c->p2_dev[ax];

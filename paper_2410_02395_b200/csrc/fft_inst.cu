@@ -26,33 +26,41 @@ constexpr int CC = MBS_CC;
 #else
 constexpr int CC = FftPlan<MBS_FFT_SIZE>::CC;
 #endif
-constexpr int NTS = PL::T * CS;
+// the kernel-multiply sweep (two FFTs per tile) may use a narrower tile than the single-FFT sweeps
+#ifdef MBS_CSM
+constexpr int CSM = MBS_CSM;
+#else
+constexpr int CSM = FftPlan<MBS_FFT_SIZE>::CSM;
+#endif
+template <int MODE> constexpr int cs_of() { return MODE == FFT_MID ? CSM : CS; }
+template <int MODE> constexpr int nts_of() { return PL::T * cs_of<MODE>(); }
 constexpr int NTC = PL::T * CC;
 
 template <int MODE>
-__global__ void __launch_bounds__(NTS) k_fft_strided(cf* __restrict__ data, const StridedGeom g, const SymbolParams sp,
+__global__ void __launch_bounds__(nts_of<MODE>()) k_fft_strided(cf* __restrict__ data, const StridedGeom g, const SymbolParams sp,
                                                     const cf* __restrict__ tw, const int* __restrict__ done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     if (done && *done) return;
-    fft_strided_body<PL, CS, MODE>(data, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
+    fft_strided_body<PL, cs_of<MODE>(), MODE>(data, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
 }
 
 // TMA-fed variant (fft_tma.cuh): persistent CTAs, NSTAGE shared-memory stages
+template <int MODE>
 constexpr int tma_stages() {
-    const size_t stage = (size_t)PL::M * CS * sizeof(cf);
+    const size_t stage = (size_t)PL::M * cs_of<MODE>() * sizeof(cf);
     const size_t budget = 220 * 1024;
     return stage * 3 <= budget ? 3 : (stage * 2 <= budget ? 2 : 0);
 }
-constexpr int NSTAGE = tma_stages();
+template <int MODE> constexpr int nstage_of() { return tma_stages<MODE>() >= 2 ? tma_stages<MODE>() : 2; }
 
 template <int MODE>
-__global__ void __launch_bounds__(NTS) k_fft_strided_tma(const __grid_constant__ CUtensorMap tmap, const StridedGeom g,
+__global__ void __launch_bounds__(nts_of<MODE>()) k_fft_strided_tma(const __grid_constant__ CUtensorMap tmap, const StridedGeom g,
                                                         const SymbolParams sp, const cf* __restrict__ tw,
                                                         const int* __restrict__ done) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     if (done && *done) return;
-    if constexpr (NSTAGE >= 2)
-        fft_strided_tma_body<PL, CS, MODE, (NSTAGE >= 2 ? NSTAGE : 2)>(&tmap, g, sp, tw, reinterpret_cast<cf*>(smem_raw));
+    if constexpr (tma_stages<MODE>() >= 2)
+        fft_strided_tma_body<PL, cs_of<MODE>(), MODE, nstage_of<MODE>()>(&tmap, g, sp, tw, reinterpret_cast<cf*>(smem_raw));
 }
 
 template <int MODE>
@@ -133,30 +141,30 @@ template <int MODE>
 cudaError_t run_strided_tma(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, const int* done,
                             int num_sms, cudaStream_t st) {
     CUtensorMap map;
-    cudaError_t e = make_strided_tensor_map(&map, data, g, PL::M, CS);
+    cudaError_t e = make_strided_tensor_map(&map, data, g, PL::M, cs_of<MODE>());
     if (e != cudaSuccess) return e;
-    const size_t smem = tma_smem_bytes<PL, CS, (NSTAGE >= 2 ? NSTAGE : 2)>();
+    const size_t smem = tma_smem_bytes<PL, cs_of<MODE>(), nstage_of<MODE>()>();
     int bps = 1;
-    e = prepare(k_fft_strided_tma<MODE>, NTS, smem, &bps);
+    e = prepare(k_fft_strided_tma<MODE>, nts_of<MODE>(), smem, &bps);
     if (e != cudaSuccess) return e;
     long long nb = (long long)num_sms * bps;
     if (nb > g.n_tiles) nb = g.n_tiles;
     if (nb < 1) return cudaSuccess;
-    k_fft_strided_tma<MODE><<<(unsigned)nb, NTS, smem, st>>>(map, g, sp, tw, done);
+    k_fft_strided_tma<MODE><<<(unsigned)nb, nts_of<MODE>(), smem, st>>>(map, g, sp, tw, done);
     return cudaGetLastError();
 }
 
 template <int MODE>
 cudaError_t run_strided(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, const int* done,
                         int num_sms, cudaStream_t st) {
-    const size_t smem = sizeof(cf) * strided_smem_elems<PL, CS>();
+    const size_t smem = sizeof(cf) * strided_smem_elems<PL, cs_of<MODE>()>();
     int bps = 1;
-    cudaError_t e = prepare(k_fft_strided<MODE>, NTS, smem, &bps);
+    cudaError_t e = prepare(k_fft_strided<MODE>, nts_of<MODE>(), smem, &bps);
     if (e != cudaSuccess) return e;
     long long nb = (long long)num_sms * bps;
     if (nb > g.n_tiles) nb = g.n_tiles;
     if (nb < 1) return cudaSuccess;
-    k_fft_strided<MODE><<<(unsigned)nb, NTS, smem, st>>>(data, g, sp, tw, done);
+    k_fft_strided<MODE><<<(unsigned)nb, nts_of<MODE>(), smem, st>>>(data, g, sp, tw, done);
     return cudaGetLastError();
 }
 
@@ -343,12 +351,10 @@ int line_blocks_entry(int mode, int t, long long n_lines, int num_sms) {
 cudaError_t strided_entry(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, int mode,
                           const int* done, int num_sms, int use_tma, cudaStream_t st) {
     // TMA needs 16-byte multiples for the global strides (inner even) and a 16-byte aligned base
-    if (use_tma && NSTAGE >= 2 && g.inner % 2 == 0 && (reinterpret_cast<uintptr_t>(data) & 15) == 0) {
-        switch (mode) {
-            case FFT_FWD: return run_strided_tma<FFT_FWD>(data, g, sp, tw, done, num_sms, st);
-            case FFT_INV: return run_strided_tma<FFT_INV>(data, g, sp, tw, done, num_sms, st);
-            default: return run_strided_tma<FFT_MID>(data, g, sp, tw, done, num_sms, st);
-        }
+    if (use_tma && g.inner % 2 == 0 && (reinterpret_cast<uintptr_t>(data) & 15) == 0) {
+        if (mode == FFT_FWD && tma_stages<FFT_FWD>() >= 2) return run_strided_tma<FFT_FWD>(data, g, sp, tw, done, num_sms, st);
+        if (mode == FFT_INV && tma_stages<FFT_INV>() >= 2) return run_strided_tma<FFT_INV>(data, g, sp, tw, done, num_sms, st);
+        if (mode == FFT_MID && tma_stages<FFT_MID>() >= 2) return run_strided_tma<FFT_MID>(data, g, sp, tw, done, num_sms, st);
     }
     switch (mode) {
         case FFT_FWD: return run_strided<FFT_FWD>(data, g, sp, tw, done, num_sms, st);
@@ -371,7 +377,7 @@ cudaError_t contig_entry(const cf* src, cf* dst, const ContigGeom& g, const Symb
 #define MBS_CAT2(a, b) a##b
 #define MBS_CAT(a, b) MBS_CAT2(a, b)
 extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {
-    MBS_FFT_SIZE, CS, CC, strided_entry, contig_entry, fused_entry, fused_blocks_entry,
+    MBS_FFT_SIZE, CS, CSM, CC, strided_entry, contig_entry, fused_entry, fused_blocks_entry,
     line_ok() ? line_entry : nullptr, line_ok() ? line_blocks_entry : nullptr,
     line_ok() ? merged_entry : nullptr, line_ok() ? merged_blocks_entry : nullptr};
 

@@ -1,5 +1,6 @@
 // fft_plans.h -- the subdomain lengths M this build has FFT plans for (2^a, 5*2^a and 3*2^a), with the
-// points per thread P, the pass radices and the lines per tile C of each.
+// points per thread P, the pass radices, the tile widths CS / CSM of the strided forward-inverse / kernel-multiply
+// sweeps (voxels per tile row) and the lines per tile CC of the contiguous tile kernels.
 // BASELINE.json configs need 128 (cfg 1, 3), 256 (cfg 3, 5), 320 (cfg 4) and 512 (cfg 2, 5).
 #pragma once
 #include "fft_core.cuh"
@@ -8,24 +9,24 @@ namespace mbs {
 
 template <int M> struct FftPlan;
 //                                          M     P   radices...
-template <> struct FftPlan<8>    { using type = Plan<8,    8,  8>;            static constexpr int CS = 64, CC = 64; };
-template <> struct FftPlan<16>   { using type = Plan<16,   8,  8, 2>;         static constexpr int CS = 64, CC = 64; };
-template <> struct FftPlan<32>   { using type = Plan<32,   8,  8, 4>;         static constexpr int CS = 32, CC = 32; };
-template <> struct FftPlan<64>   { using type = Plan<64,   8,  8, 8>;         static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<128>  { using type = Plan<128,  16, 16, 8>;        static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<256>  { using type = Plan<256,  16, 16, 16>;       static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<512>  { using type = Plan<512,  16, 16, 16, 2>;    static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<1024> { using type = Plan<1024, 16, 16, 16, 4>;    static constexpr int CS = 8, CC = 8;  };
-template <> struct FftPlan<40>   { using type = Plan<40,   20, 20, 2>;        static constexpr int CS = 64, CC = 64; };
-template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        static constexpr int CS = 32, CC = 32; };
-template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 32, CC = 16; };
-template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<48>   { using type = Plan<48,   12, 12, 4>;        static constexpr int CS = 64, CC = 64; };
-template <> struct FftPlan<96>   { using type = Plan<96,   24, 12, 8>;        static constexpr int CS = 32, CC = 32; };
-template <> struct FftPlan<192>  { using type = Plan<192,  12, 12, 4, 4>;     static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<384>  { using type = Plan<384,  24, 12, 8, 4>;     static constexpr int CS = 16, CC = 16; };
-template <> struct FftPlan<768>  { using type = Plan<768,  24, 12, 8, 8>;     static constexpr int CS = 8, CC = 8;  };
+template <> struct FftPlan<8>    { using type = Plan<8,    8,  8>;            static constexpr int CS = 64, CSM = 64, CC = 64; };
+template <> struct FftPlan<16>   { using type = Plan<16,   8,  8, 2>;         static constexpr int CS = 64, CSM = 64, CC = 64; };
+template <> struct FftPlan<32>   { using type = Plan<32,   8,  8, 4>;         static constexpr int CS = 32, CSM = 32, CC = 32; };
+template <> struct FftPlan<64>   { using type = Plan<64,   8,  8, 8>;         static constexpr int CS = 16, CSM = 16, CC = 16; };
+template <> struct FftPlan<128>  { using type = Plan<128,  16, 16, 8>;        static constexpr int CS = 16, CSM = 16, CC = 16; };
+template <> struct FftPlan<256>  { using type = Plan<256,  16, 16, 16>;       static constexpr int CS = 32, CSM = 16, CC = 16; };
+template <> struct FftPlan<512>  { using type = Plan<512,  16, 16, 16, 2>;    static constexpr int CS = 16, CSM = 16, CC = 16; };
+template <> struct FftPlan<1024> { using type = Plan<1024, 16, 16, 16, 4>;    static constexpr int CS = 8, CSM = 8, CC = 8;  };
+template <> struct FftPlan<40>   { using type = Plan<40,   20, 20, 2>;        static constexpr int CS = 64, CSM = 64, CC = 64; };
+template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        static constexpr int CS = 32, CSM = 32, CC = 32; };
+template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int CS = 16, CSM = 16, CC = 16; };
+template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 32, CSM = 32, CC = 16; };
+template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int CS = 16, CSM = 16, CC = 16; };
+template <> struct FftPlan<48>   { using type = Plan<48,   12, 12, 4>;        static constexpr int CS = 64, CSM = 64, CC = 64; };
+template <> struct FftPlan<96>   { using type = Plan<96,   24, 12, 8>;        static constexpr int CS = 32, CSM = 32, CC = 32; };
+template <> struct FftPlan<192>  { using type = Plan<192,  12, 12, 4, 4>;     static constexpr int CS = 16, CSM = 16, CC = 16; };
+template <> struct FftPlan<384>  { using type = Plan<384,  24, 12, 8, 4>;     static constexpr int CS = 16, CSM = 16, CC = 16; };
+template <> struct FftPlan<768>  { using type = Plan<768,  24, 12, 8, 8>;     static constexpr int CS = 8, CSM = 8, CC = 8;  };
 
 }  // namespace mbs
 

@@ -159,7 +159,7 @@ static void report(const char* what, int M, double err) {
 template <int M>
 static void test_size() {
     using PL = typename FftPlan<M>::type;
-    constexpr int CS = FftPlan<M>::CS, CC = FftPlan<M>::CC;
+    constexpr int CS = FftPlan<M>::CSM, CC = FftPlan<M>::CC;
     report("strided fwd", M, test_strided<PL, CS, FFT_FWD>(2, 2, CS + 5));
     report("strided inv", M, test_strided<PL, CS, FFT_INV>(1, 2, CS + 5));
     report("strided mid", M, test_strided<PL, CS, FFT_MID>(1, 1, CS + 3));

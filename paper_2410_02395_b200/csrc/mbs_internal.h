@@ -178,7 +178,8 @@ struct FusedParams {
 // FFT registry (fft_inst.cu compiled once per size, fft_registry.cu)
 struct FftEntry {
     int M;
-    int CS;  // voxels per tile row of the strided sweeps
+    int CS;  // voxels per tile row of the strided forward / inverse sweeps
+    int CSM; // voxels per tile row of the strided kernel-multiply sweep
     int CC;  // lines per tile of the contiguous sweeps
     cudaError_t (*strided)(cf* data, const StridedGeom& g, const SymbolParams& sp, const cf* tw, int mode,
                            const int* done, int num_sms, int use_tma, cudaStream_t st);
