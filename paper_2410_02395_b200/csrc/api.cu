@@ -220,6 +220,15 @@ static double sigma_max(const std::vector<double>& K, int t) {
 // ---------------------------------------------------------------------------------------------
 static size_t align_up(size_t v, size_t a = 256) { return (v + a - 1) / a * a; }
 
+// A captured graph holds the device pointers of the launches it recorded: drop it whenever one of them changes
+// (workspace, residual-history buffer).
+static void invalidate_graph(mbs_ctx* c) {
+    if (c->graph_exec) {
+        cudaGraphExecDestroy(c->graph_exec);
+        c->graph_exec = nullptr;
+    }
+}
+
 static size_t corr_elems(const GridDesc& g, int ax) {
     if (g.a[ax] == 0 || g.t == 0) return 0;
     return (size_t)(g.voxels / g.N[ax]) * g.S[ax] * 2 * g.t;
@@ -417,6 +426,7 @@ extern "C" int mbs_set_workspace(mbs_ctx* c, void* device_buffer, size_t bytes) 
     if (!device_buffer || bytes < c->ws_bytes) return fail(c, MBS_ERR_INVALID_ARG, "workspace needs %zu bytes, got %zu", c->ws_bytes, bytes);
     if (((uintptr_t)device_buffer & 255) != 0) return fail(c, MBS_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
     if (c->ws_owned && c->ws) cudaFree(c->ws);
+    invalidate_graph(c);
     c->ws = device_buffer;
     c->ws_owned = false;
     layout_workspace(c, (char*)c->ws);
@@ -831,6 +841,7 @@ static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, do
 
 static int ensure_history(mbs_ctx* c, int32_t max_iter) {
     if (c->hist_cap < max_iter) {
+        invalidate_graph(c);
         if (c->hist_dev) cudaFree(c->hist_dev);
         c->hist_dev = nullptr;
         c->hist_cap = 0;

@@ -413,3 +413,27 @@ def test_operators_and_first_residuals_mid_size(B, orc, name, make):
     assert np.allclose(hist, h_ref, rtol=1e-4), (hist, h_ref)
     assert rel(xd.cpu().numpy(), x_ref) <= OP_TOL
     s.close()
+
+
+def test_graph_reuse_across_solves(B):
+    """Small grids replay CUDA graphs of a poll interval.  The graph is reused while the arrays stay the same and must
+    be rebuilt when a recorded buffer changes (here: the residual-history buffer grows with max_iter)."""
+    import torch
+    w = workloads.config(2, shape=(128, 128), boundary_width=(8, 8))
+    n, y = w.make_medium(), w.make_source()
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    yd = torch.from_numpy(y).cuda()
+    xd = torch.zeros(w.shape, dtype=torch.complex64, device="cuda")
+    rc, h1, n1 = B.mbs_solve(s.ctx, yd.data_ptr(), xd.data_ptr(), 0.0, 200)      # several graph replays
+    xd.zero_()
+    rc, h2, n2 = B.mbs_solve(s.ctx, yd.data_ptr(), xd.data_ptr(), 0.0, 700)      # same arrays, larger history buffer
+    x2 = xd.clone()
+    assert n1 == 200 and n2 == 700 and np.array_equal(h2[:200], h1)
+    s2 = B.Solver.from_workload(w)
+    s2.set_option(B.MBS_OPT_USE_GRAPH, 0)
+    s2.set_potential(n)
+    x3, h3, rc3 = s2.solve(y, tol=0.0, max_iter=700)
+    assert np.array_equal(h3, h2) and torch.equal(x3, x2)
+    s.close()
+    s2.close()
