@@ -465,6 +465,8 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
 extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
     if (!c) return MBS_ERR_INVALID_ARG;
     if (!n_map_device) return fail(c, MBS_ERR_INVALID_ARG, "n_map is NULL");
+    invalidate_graph(c);                              // the scale factor c is recorded by value in the launches
+    c->potential_set = false;
     MBS_TRY(ensure_workspace(c));
     const GridDesc& g = c->g;
     SetupParams sp{};

@@ -435,5 +435,13 @@ def test_graph_reuse_across_solves(B):
     s2.set_potential(n)
     x3, h3, rc3 = s2.solve(y, tol=0.0, max_iter=700)
     assert np.array_equal(h3, h2) and torch.equal(x3, x2)
+    # a new medium changes the scale factor c that the recorded launches carry by value
+    n_b = workloads.random_medium(w.shape, 77, 1.0, 1.4, 0.01)
+    s.set_potential(n_b)
+    s2.set_potential(n_b)
+    xd.zero_()
+    rc, h4, n4 = B.mbs_solve(s.ctx, yd.data_ptr(), xd.data_ptr(), 0.0, 300)
+    x5, h5, rc5 = s2.solve(y, tol=0.0, max_iter=300)
+    assert np.array_equal(h4, h5) and torch.equal(x5, xd)
     s.close()
     s2.close()
