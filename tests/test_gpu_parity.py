@@ -92,6 +92,9 @@ ITERATION_CASES = OPERATOR_CASES + [
     ((8, 8, 256), (1, 1, 2), (0, 0, 8), 8, (1, 1, 0)),       # periodic single-domain axes 0, 1: no slab rows
     ((48, 40, 64), (3, 1, 2), (4, 4, 4), 8, None),            # ragged tile tail: 48*40*2 lines is not a multiple of 16
     ((32, 32, 320), (2, 2, 1), (4, 4, 8), 8, None),
+    ((1024,), (1,), (16,), 8, None),                           # longest plan: a line spans two warps -> tile kernels
+    ((16, 2048), (1, 2), (4, 16), 8, None),
+    ((1024, 40), (1, 1), (16, 0), 8, (0, 1)),                  # 1024-long strided lines, ragged tile tail (40 columns)
     ((768,), (1,), (16,), 8, None),                            # 3 * 2^k line lengths
     ((384,), (2,), (8,), 8, None),
     ((96, 48), (1, 1), (4, 4), 8, None),
