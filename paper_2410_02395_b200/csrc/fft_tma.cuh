@@ -125,13 +125,6 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
     for (unsigned i = 0; i < n_mine; ++i) {
         const int s = (int)(i % NSTAGE);
         cf* tile = stage0 + (size_t)s * M * C;
-        if constexpr (NSTAGE < 3) {
-            if (tid == 0 && i + NSTAGE - 1 < n_mine) {
-                // the stage of tile i-1 is refilled: its store must have finished reading shared memory
-                tma_wait_read<0>();
-                issue_load(i + NSTAGE - 1);
-            }
-        }
         int c0, c1, c2, ii0;
         coords(i, c0, c1, c2, ii0);
         // |p|^2 of the other axes for this thread's line: requested before the wait so its latency is covered
@@ -156,7 +149,22 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
             static_for<0, P>([&](auto mc) { v[decltype(mc)::value] = cswap(v[decltype(mc)::value]); });
         }
         fft_line_forward<PL, C, 1>(v, tile, c, jt, tw);
+        if constexpr (NSTAGE < 3 && MODE != FFT_MID) {
+            // two stages: refill the other one after the butterflies of this tile (see the kernel-multiply case below)
+            if (tid == 0 && i + NSTAGE - 1 < n_mine) {
+                tma_wait_read<0>();
+                issue_load(i + NSTAGE - 1);
+            }
+        }
         if constexpr (MODE == FFT_MID) {
+            if constexpr (NSTAGE < 3) {
+                // two stages: refill the other one between the two FFTs of this tile; by now the store of the tile
+                // before has long finished reading it, so the elected thread does not hold the CTA back
+                if (tid == 0 && i + NSTAGE - 1 < n_mine) {
+                    tma_wait_read<0>();
+                    issue_load(i + NSTAGE - 1);
+                }
+            }
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
                 v[m] = cswap(apply_symbol(v[m], p2a[m] + wline, sp));
