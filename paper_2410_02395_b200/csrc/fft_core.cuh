@@ -317,8 +317,25 @@ constexpr int line_scratch_elems() { return PL::M + PL::M / 16 + 1; }
 
 MBS_DEV int pad16(int i) { return i + (i >> 4); }
 
+// Twiddles of the warp-local variant.  Lanes of a warp hold consecutive points of ONE line, so for a fixed butterfly
+// input r they need W^{r k} for consecutive k: the table is laid out per pass as [r - 1][k] (k fastest), which makes
+// those reads unit-stride (the natural table W_M^n would be read with stride 2 r ... 16 r: up to 16-way bank
+// conflicts).  Pass i > 0 starts at Ns_i - Ns_1 (the sizes (R_i - 1) Ns_i telescope), total M - R_0 < M entries.
 template <class PL>
-MBS_DEV void fft_line_forward_warp(cf (&v)[PL::P], cf* line, const int jt, const cf* MBS_RESTRICT tw) {
+MBS_DEV void fill_warp_twiddles(cf* twp, const cf* MBS_RESTRICT tw_global, const int tid, const int nthreads) {
+    constexpr int M = PL::M;
+    static_for<1, PL::NPASS>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int R = PL::radix(i), Ns = PL::ns(i), base = Ns - PL::ns(1);
+        for (int idx = tid; idx < (R - 1) * Ns; idx += nthreads) {
+            const int r = idx / Ns + 1, k = idx - (r - 1) * Ns;
+            twp[base + idx] = tw_global[r * k * (M / (Ns * R))];
+        }
+    });
+}
+
+template <class PL>
+MBS_DEV void fft_line_forward_warp(cf (&v)[PL::P], cf* line, const int jt, const cf* MBS_RESTRICT twp) {
     constexpr int M = PL::M, P = PL::P, T = PL::T;
     static_assert(T <= 32, "a line must fit in one warp");
     static_for<0, PL::NPASS>([&](auto ic) {
@@ -332,10 +349,10 @@ MBS_DEV void fft_line_forward_warp(cf (&v)[PL::P], cf* line, const int jt, const
                 constexpr int b = decltype(bc)::value;
                 const int j = jt + b * T;
                 const int k = j % Ns;
-                const int step = k * (M / (Ns * R));
+                constexpr int base = Ns - PL::ns(1);
                 static_for<1, R>([&](auto rc) {
                     constexpr int r = decltype(rc)::value;
-                    v[b + r * NB] = cmul(v[b + r * NB], tw[r * step]);
+                    v[b + r * NB] = cmul(v[b + r * NB], twp[base + (r - 1) * Ns + k]);
                 });
             });
         }

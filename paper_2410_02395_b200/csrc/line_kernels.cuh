@@ -130,7 +130,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
     cf* tw = smem;
     cf* scratch = tw + M + (warp * LW + lane / T) * LSE;
     float* Ks = reinterpret_cast<float*>(tw + M + NWARP * LW * LSE);
-    for (int i = tid; i < M; i += NT) tw[i] = tw_global[i];
+    fill_warp_twiddles<PL>(tw, tw_global, tid, NT);   // per-pass [r][k] layout: conflict-free for lanes along a line
     if (p.a2) for (int i = tid; i < t * t; i += NT) Ks[i] = p.Kh[i];
     __syncthreads();
     const int jt = lane % T, lsub = lane / T;
