@@ -518,12 +518,23 @@ static cf to_cf(cd z) { return make_float2((float)z.real(), (float)z.imag()); }
 
 // edge corrections of (in - in2) into c->cx  (a2 / a7 of the scope table)
 static int run_slabs(mbs_ctx* c, const cf* in, const cf* in2, bool in_loop, int axis_mask = 7, bool from_ds = false) {
-    for (int ax = 0; ax < 3; ++ax) {
-        if (!c->cx.buf[ax] || !((axis_mask >> ax) & 1)) continue;
+    auto params = [&](int ax) {
         SlabParams sp{};
         sp.in = from_ds ? c->ds.buf[ax] : in; sp.in2 = in2; sp.out = c->cx.buf[ax]; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
         sp.compact_in = from_ds ? 1 : 0;
         sp.state = c->state; sp.check_done = in_loop ? 1 : 0;
+        return sp;
+    };
+    if (c->cx.buf[0] && c->cx.buf[1] && (axis_mask & 3) == 3 && slab_pair_supported(c->g.t)) {
+        // axes 0 and 1 in one launch
+        const SlabParams pA = params(0), pB = params(1);
+        KernelScope ks(c, "slab_ax01", (in2 ? 24.0 : 16.0) * ((double)corr_elems(c->g, 0) + (double)corr_elems(c->g, 1)));
+        MBS_CUDA(c, launch_slab_pair(c->g, pA, pB, c->stream));
+        axis_mask &= ~3;
+    }
+    for (int ax = 0; ax < 3; ++ax) {
+        if (!c->cx.buf[ax] || !((axis_mask >> ax) & 1)) continue;
+        const SlabParams sp = params(ax);
         static const char* names[3] = {"slab_ax0", "slab_ax1", "slab_ax2"};
         KernelScope ks(c, names[ax], (in2 ? 24.0 : 16.0) * (double)corr_elems(c->g, ax));
         MBS_CUDA(c, launch_slab(c->g, sp, c->stream));

@@ -45,16 +45,29 @@ __global__ void __launch_bounds__(nts_of<MODE>()) k_fft_strided(cf* __restrict__
 }
 
 // TMA-fed variant (fft_tma.cuh): persistent CTAs, NSTAGE shared-memory stages
+template <class F, class = void> struct plan_nstage { static constexpr int value = 0; };
+template <class F> struct plan_nstage<F, std::void_t<decltype(F::NSTAGE)>> { static constexpr int value = F::NSTAGE; };
 template <int MODE>
 constexpr int tma_stages() {
     const size_t stage = (size_t)PL::M * cs_of<MODE>() * sizeof(cf);
     const size_t budget = 220 * 1024;
+#ifdef MBS_NSTAGE_MID
+    if (MODE == FFT_MID) return stage * MBS_NSTAGE_MID <= budget ? MBS_NSTAGE_MID : 0;
+#endif
+#ifdef MBS_NSTAGE
+    if (MODE != FFT_MID) return stage * MBS_NSTAGE <= budget ? MBS_NSTAGE : 0;
+#endif
+    constexpr int fixed = plan_nstage<FftPlan<MBS_FFT_SIZE>>::value;
+    if (MODE != FFT_MID && fixed >= 2 && stage * fixed <= budget) return fixed;
     return stage * 3 <= budget ? 3 : (stage * 2 <= budget ? 2 : 0);
 }
 template <int MODE> constexpr int nstage_of() { return tma_stages<MODE>() >= 2 ? tma_stages<MODE>() : 2; }
 
+#ifndef MBS_MID_MINB
+#define MBS_MID_MINB 1
+#endif
 template <int MODE>
-__global__ void __launch_bounds__(nts_of<MODE>()) k_fft_strided_tma(const __grid_constant__ CUtensorMap tmap, const StridedGeom g,
+__global__ void __launch_bounds__(nts_of<MODE>(), MODE == FFT_MID ? MBS_MID_MINB : 1) k_fft_strided_tma(const __grid_constant__ CUtensorMap tmap, const StridedGeom g,
                                                         const SymbolParams sp, const cf* __restrict__ tw,
                                                         const int* __restrict__ done) {
     extern __shared__ __align__(128) unsigned char smem_raw[];

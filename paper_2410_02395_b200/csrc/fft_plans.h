@@ -1,6 +1,8 @@
 // fft_plans.h -- the subdomain lengths M this build has FFT plans for (2^a, 5*2^a and 3*2^a), with the
 // points per thread P, the pass radices, the tile widths CS / CSM of the strided forward-inverse / kernel-multiply
-// sweeps (voxels per tile row) and the lines per tile CC of the contiguous tile kernels.
+// sweeps (voxels per tile row) and the lines per tile CC of the contiguous tile kernels.  An optional NSTAGE fixes
+// the TMA stages of the forward/inverse strided sweeps (default: as many as fit, at most 3); 320 runs two 40 KiB
+// stages so that two CTAs share an SM (measured on cfg 4: 0.77 ms against 0.86 ms with one CTA of 32-wide tiles).
 // BASELINE.json configs need 128 (cfg 1, 3), 256 (cfg 3, 5), 320 (cfg 4) and 512 (cfg 2, 5).
 #pragma once
 #include "fft_core.cuh"
@@ -20,7 +22,7 @@ template <> struct FftPlan<1024> { using type = Plan<1024, 16, 16, 16, 4>;    st
 template <> struct FftPlan<40>   { using type = Plan<40,   20, 20, 2>;        static constexpr int CS = 64, CSM = 64, CC = 64; };
 template <> struct FftPlan<80>   { using type = Plan<80,   20, 20, 4>;        static constexpr int CS = 32, CSM = 32, CC = 32; };
 template <> struct FftPlan<160>  { using type = Plan<160,  20, 20, 4, 2>;     static constexpr int CS = 16, CSM = 16, CC = 16; };
-template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 32, CSM = 32, CC = 16; };
+template <> struct FftPlan<320>  { using type = Plan<320,  20, 20, 4, 4>;     static constexpr int CS = 16, CSM = 32, CC = 16, NSTAGE = 2; };
 template <> struct FftPlan<640>  { using type = Plan<640,  20, 20, 4, 4, 2>;  static constexpr int CS = 16, CSM = 16, CC = 16; };
 template <> struct FftPlan<48>   { using type = Plan<48,   12, 12, 4>;        static constexpr int CS = 64, CSM = 64, CC = 64; };
 template <> struct FftPlan<96>   { using type = Plan<96,   24, 12, 8>;        static constexpr int CS = 32, CSM = 32, CC = 32; };

@@ -101,6 +101,8 @@ struct FixupParams {
 // launchers implemented in kernels.cu
 cudaError_t launch_pointwise(const GridDesc& g, const PointwiseParams& p, int num_sms, cudaStream_t st);
 cudaError_t launch_slab(const GridDesc& g, const SlabParams& p, cudaStream_t st);
+bool slab_pair_supported(int t);   // launch_slab_pair: two axes in one launch (t = 2, 4, 8, 16)
+cudaError_t launch_slab_pair(const GridDesc& g, const SlabParams& pA, const SlabParams& pB, cudaStream_t st);
 // slab pass of one axis (kernels.cu: k_slab_pass): corr_ax(d) from the compact d, applied to u / x in the same kernel
 struct SlabPassParams {
     const cf* ds;      // compact d of this axis, [outer][S*2t][inner]
