@@ -245,7 +245,7 @@ cudaError_t line_grid(int t, long long n_lines, int num_sms, int* nb_out, size_t
     if constexpr (!line_ok()) {
         return cudaErrorNotSupported;
     } else {
-        const size_t smem = line_smem_bytes<PL, LINE_WARPS>(t);
+        const size_t smem = line_smem_bytes<PL, LINE_WARPS, MODE>(t);
         int bps = 1;
         cudaError_t e = prepare(k_line<MODE>, LINE_WARPS * 32, smem, &bps);
         if (e != cudaSuccess) return e;

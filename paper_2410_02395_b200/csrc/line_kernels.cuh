@@ -21,10 +21,23 @@
 
 namespace mbs {
 
-template <class PL, int NWARP>
+// Plans with more than 16 points per thread (5 * 2^a and 3 * 2^a sizes) cannot hold u, x AND B_diag of a line in 128
+// registers across the FFT of the last sweep: there B_diag of the line is requested with cp.async into a per-line stage
+// in shared memory before the butterflies (no registers, no spills) and read back after them.
+template <class PL, int MODE>
+constexpr bool line_stage_b() { return MODE == LINE_S5 && PL::P > 16; }
+template <class PL, int NWARP, int MODE = LINE_S1>
 constexpr size_t line_smem_bytes(int t) {
-    return sizeof(cf) * (size_t)(PL::M + NWARP * (32 / PL::T) * line_scratch_elems<PL>()) + sizeof(float) * (size_t)(t * t) + 16;
+    return sizeof(cf) * (size_t)(PL::M + NWARP * (32 / PL::T) * line_scratch_elems<PL>() +
+                                 (line_stage_b<PL, MODE>() ? NWARP * 32 * PL::P + 2 : 0)) +
+           sizeof(float) * (size_t)(t * t) + 16;
 }
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 __device__ __forceinline__ int line_edge_slot(int i, int M, int t) {   // as fused_edge_slot: s*2t + e, or -1
     const int s = i / M, e = i - s * M;
@@ -129,7 +142,10 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
     const int t = p.t, t2 = 2 * p.t;
     cf* tw = smem;
     cf* scratch = tw + M + (warp * LW + lane / T) * LSE;
-    float* Ks = reinterpret_cast<float*>(tw + M + NWARP * LW * LSE);
+    constexpr bool STAGE_B = line_stage_b<PL, MODE>();
+    constexpr int BST0 = (M + NWARP * LW * LSE + 1) & ~1;              // 16-byte aligned start of the B_diag stages
+    cf* bst = tw + BST0 + (warp * LW + lane / T) * M;                  // this line's stage (STAGE_B only)
+    float* Ks = reinterpret_cast<float*>(tw + (STAGE_B ? BST0 + NWARP * LW * M : M + NWARP * LW * LSE));
     fill_warp_twiddles<PL>(tw, tw_global, tid, NT);   // per-pass [r][k] layout: conflict-free for lanes along a line
     if (p.a2) for (int i = tid; i < t * t; i += NT) Ks[i] = p.Kh[i];
     __syncthreads();
@@ -204,7 +220,16 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                 v[m] = valid ? cswap(p.u[gl + jt + m * T]) : make_float2(0.f, 0.f);
             });
             // x and B_diag of the line are requested before the butterflies, so their HBM latency is covered
-            constexpr bool PREFETCH_B = true;   // measured: also for 20 points per thread the early request wins over the spills it costs
+            constexpr bool PREFETCH_B = !STAGE_B;
+            if constexpr (STAGE_B) {
+                __syncwarp();                                          // the stage is no longer read by the unit before
+                if (valid) {
+                    const cf* src = p.bdiag + gl;
+#pragma unroll
+                    for (int i = 0; i < P / 2; ++i) cp_async16(bst + 2 * (jt + i * T), src + 2 * (jt + i * T));
+                }
+                cp_async_commit();
+            }
             cf xr[P], br[PREFETCH_B ? P : 1];
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
@@ -212,6 +237,10 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                 if constexpr (PREFETCH_B) br[m] = valid ? p.bdiag[gl + jt + m * T] : make_float2(0.f, 0.f);
             });
             fft_line_forward_warp<PL>(v, scratch, jt, tw);
+            if constexpr (STAGE_B) {
+                cp_async_wait_all();
+                __syncwarp();                                          // every lane's copies have landed
+            }
             if (valid) {
                 const bool slab_row = (o0 >= 0) || (o1 >= 0);
                 const long long o2 = (long long)row * (p.S2 * t2) + (long long)seg * t2;
@@ -222,7 +251,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                     const cf d = csub(xv, cswap(v[m]));
                     cf bv;
                     if constexpr (PREFETCH_B) bv = br[m];
-                    else bv = p.bdiag[gl + pidx];
+                    else bv = bst[pidx];
                     const cf r = cmul(bv, d);
                     const bool edge2 = p.a2 && (pidx < t || pidx >= M - t);
                     if (!slab_row && !edge2) {
