@@ -36,6 +36,7 @@ constexpr size_t line_smem_bytes(int t) {
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void* gptr) { asm volatile("prefetch.global.L2 [%0];" ::"l"(gptr)); }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -207,6 +208,21 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                     if (pidx < t || pidx >= M - t) v[m] = csub(v[m], line_corr2_x<M>(p, Ks, grow, seg, pidx));
                 });
             }
+#ifndef MBS_NO_L2_PREFETCH
+            // x and B_diag of the line this warp takes next are requested into L2 now (one 128-byte line per lane and
+            // request: no registers, no shared memory), so that their loads after this FFT are L2 hits
+            if (!p.slab_rows_only) {
+                const unsigned nline = (unit + gridDim.x * NWARP) * LW + lsub;
+                if (nline < n_lines) {
+                    const char* nx = reinterpret_cast<const char*>(p.x + (long long)nline * M);
+                    const char* nb = reinterpret_cast<const char*>(p.bdiag + (long long)nline * M);
+                    for (int off = jt * 128; off < M * (int)sizeof(cf); off += T * 128) {
+                        prefetch_l2(nx + off);
+                        prefetch_l2(nb + off);
+                    }
+                }
+            }
+#endif
             fft_line_forward_warp<PL>(v, scratch, jt, tw);
             if (valid) {
                 static_for<0, P>([&](auto mc) {
