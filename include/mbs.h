@@ -107,7 +107,9 @@ typedef struct mbs_info {
 /*
  * Create a solver for one grid (P:37-45 problem statement; P:82 decomposition).
  *  ndim            1, 2 or 3.
- *  shape[ndim]     grid size in voxels INCLUDING the absorbing layers, axis 0 slowest.
+ *  shape[ndim]     grid size in voxels INCLUDING the absorbing layers, axis 0 slowest.  The grid may hold at most
+ *                  2^31 - 1 voxels (32-bit tile and line counters in the kernels): 1260^3 fits, 1290^3 does not
+ *                  -> MBS_ERR_INVALID_ARG.
  *  pixel_size      grid pitch h (same on every axis), same unit as wavelength.   (lambda/4)
  *  wavelength      vacuum wavelength lambda; k(r) = 2 pi n(r) / lambda.
  *  boundary_width[ndim]  W_d: thickness in voxels of the absorbing layer on each side (R3).

@@ -15,8 +15,7 @@ from typing import Optional, Sequence, Tuple
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-# MBS_B200_LIB lets a developer load another build of the same library (kernel tuning); default: in-tree
-LIB_PATH = os.environ.get("MBS_B200_LIB") or os.path.join(_HERE, "libmbs_b200.so")
+LIB_PATH = os.path.join(_HERE, "libmbs_b200.so")      # the in-tree build; no environment override
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(
@@ -236,26 +235,38 @@ class Solver:
                    periodic=w.periodic_flags(), n_correction=w.n_correction, device=device, stream=stream)
 
     def _dev(self, a):
+        """complex64 device tensor of the grid shape.  Copies and conversions are enqueued on the solver's stream, so
+        the library's kernels (same stream) are ordered after them; a tensor that is already right is passed through
+        (the caller orders its producer with the solver's stream, as with any CUDA library)."""
         torch = self._torch
         if not isinstance(a, torch.Tensor):
             a = torch.from_numpy(np.ascontiguousarray(a))
-        a = a.to(device=self.device, dtype=torch.complex64).contiguous()
+        with torch.cuda.stream(self.stream):
+            a = a.to(device=self.device, dtype=torch.complex64).contiguous()
         assert tuple(a.shape) == self.shape, (tuple(a.shape), self.shape)
         return a
+
+    def _sync(self):
+        """Temporaries created by this wrapper are released to torch's caching allocator on return; the library's
+        asynchronous kernels may still read them, so the wrapper waits for the stream first."""
+        self.stream.synchronize()
 
     def set_option(self, option: int, value: int):
         mbs_set_option(self.ctx, option, value)
 
     def set_potential(self, n_map):
         n = self._dev(n_map)
-        mbs_set_potential(self.ctx, n.data_ptr())
+        mbs_set_potential(self.ctx, n.data_ptr())       # synchronises the stream itself (include/mbs.h)
 
     def apply_operator(self, which: int, inp, out=None):
         torch = self._torch
         a = self._dev(inp)
         if out is None:
-            out = torch.empty_like(a)
+            with torch.cuda.stream(self.stream):
+                out = torch.empty_like(a)
         mbs_apply_operator(self.ctx, which, a.data_ptr(), out.data_ptr())
+        if a is not inp:
+            self._sync()                                # `a` is a temporary of this call
         return out
 
     def solve(self, y, x0=None, tol: float = 1e-6, max_iter: int = 1000):
@@ -266,8 +277,11 @@ class Solver:
             with torch.cuda.stream(self.stream):
                 xd = torch.zeros(self.shape, dtype=torch.complex64, device=self.device)
         else:
-            xd = self._dev(x0).clone()
-        rc, hist, _ = mbs_solve(self.ctx, yd.data_ptr(), xd.data_ptr(), tol, max_iter)
+            xd = self._dev(x0)
+            if xd is x0:
+                with torch.cuda.stream(self.stream):
+                    xd = xd.clone()
+        rc, hist, _ = mbs_solve(self.ctx, yd.data_ptr(), xd.data_ptr(), tol, max_iter)   # returns after a stream sync
         return xd, hist, rc
 
     def solve_host(self, y_host, x_host, tol: float, max_iter: int):

@@ -31,14 +31,27 @@ def fft_sizes():
     return [int(m) for m in re.findall(r"X\((\d+)\)", body)]
 
 
-def _source_digest():
+_INC = re.compile(r'^\s*#\s*include\s*"([^"]+)"', re.M)
+
+
+def _deps(path, seen=None):
+    """The file and every header it includes with quotes, recursively (paths relative to the including file)."""
+    seen = set() if seen is None else seen
+    path = os.path.normpath(path)
+    if path in seen or not os.path.exists(path):
+        return seen
+    seen.add(path)
+    for inc in _INC.findall(open(path).read()):
+        _deps(os.path.join(os.path.dirname(path), inc), seen)
+    return seen
+
+
+def _job_digest(src, extra):
     h = hashlib.sha256()
-    for d in (CSRC, os.path.join(ROOT, "include")):
-        for name in sorted(os.listdir(d)):
-            if name.endswith((".cu", ".cuh", ".h")):
-                h.update(name.encode())
-                h.update(open(os.path.join(d, name), "rb").read())
-    h.update(" ".join(FLAGS).encode())
+    for dep in sorted(_deps(src)):
+        h.update(os.path.relpath(dep, ROOT).encode())
+        h.update(open(dep, "rb").read())
+    h.update(" ".join(FLAGS + extra).encode())
     return h.hexdigest()
 
 
@@ -52,27 +65,34 @@ def _compile(job):
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compiles what changed (one digest per object over the source, the headers it includes and the flags) and links."""
     os.makedirs(OBJDIR, exist_ok=True)
-    stamp = os.path.join(OBJDIR, "digest.txt")
-    digest = _source_digest()
-    if not force and os.path.exists(LIB) and os.path.exists(stamp) and open(stamp).read() == digest:
-        return LIB
     jobs = []
     for name in ("api.cu", "kernels.cu", "fft_registry.cu"):
         jobs.append((os.path.join(CSRC, name), os.path.join(OBJDIR, name[:-3] + ".o"), []))
     for m in fft_sizes():
         jobs.append((os.path.join(CSRC, "fft_inst.cu"), os.path.join(OBJDIR, "fft_%d.o" % m),
                      ["-DMBS_FFT_SIZE=%d" % m]))
+    stale, digests = [], {}
+    for src, obj, extra in jobs:
+        digests[obj] = _job_digest(src, extra)
+        stamp = obj + ".digest"
+        if force or not os.path.exists(obj) or not os.path.exists(stamp) or open(stamp).read() != digests[obj]:
+            stale.append((src, obj, extra))
+    if not stale and os.path.exists(LIB):
+        return LIB
     with concurrent.futures.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
-        objs = list(ex.map(_compile, jobs))
+        list(ex.map(_compile, stale))
+    for _, obj, _ in stale:
+        with open(obj + ".digest", "w") as f:
+            f.write(digests[obj])
+    objs = [obj for _, obj, _ in jobs]
     cmd = [NVCC, "-shared", "-o", LIB] + objs + ["-Xcompiler", "-fPIC", "-lcudart"]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("link failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
-    with open(stamp, "w") as f:
-        f.write(digest)
     if verbose:
-        print("built", LIB)
+        print("built %s (%d of %d objects recompiled)" % (LIB, len(stale), len(jobs)))
     return LIB
 
 

@@ -1,5 +1,5 @@
 // compat.h -- lets the kernel bodies compile both under nvcc (device code, the product) and under a
-// plain host C++ compiler (csrc/host_emulation_test.cpp: one std::thread per CUDA thread, used only
+// plain host C++ compiler (tests/host_emulation_test.cpp: one std::thread per CUDA thread, used only
 // to check index arithmetic on a machine without a GPU; it is not a CPU fallback and is not linked
 // into the library).
 #pragma once

@@ -691,6 +691,9 @@ __global__ void __launch_bounds__(256) k_setup(const GridDesc g, const SetupPara
         double im_n;
         const double2 k2 = k2_at(g, p, idx, &im_n);
         if (pass == 0) {
+            // fmin / fmax drop a NaN operand: a non-finite voxel of n is carried explicitly as +inf in the maximum of
+            // Re k^2, which mbs_set_potential rejects (MBS_ERR_NUMERIC)
+            if (!isfinite(k2.x) || !isfinite(k2.y)) mx_re = CUDART_INF;
             mn_re = fmin(mn_re, k2.x); mx_re = fmax(mx_re, k2.x);
             mn_im = fmin(mn_im, k2.y); mx_im = fmax(mx_im, k2.y);
             mn_n = fmin(mn_n, im_n);

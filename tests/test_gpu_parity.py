@@ -3,6 +3,8 @@ element by element on the same seeded inputs.  Bars (BASELINE.json north_star): 
 <= 1e-5 per operator application; <= 1e-4 on the converged field at the same stopping threshold;
 iteration counts +-1.
 """
+import dataclasses
+
 import numpy as np
 import pytest
 
@@ -35,6 +37,56 @@ def rel(a, b):
     return float(np.linalg.norm(a - b) / np.linalg.norm(b))
 
 
+def edge_masks(shape, S, t, periodic=None):
+    """(slab, multi): voxels that are one of the 2t edge points of a subdomain along at least one axis with
+    corrections (a_d > 0), and those that are edge points along two or three such axes (where the
+    slab passes hand a voxel from one axis to the next)."""
+    D = len(shape)
+    per = periodic if periodic is not None else (0,) * D
+    count = np.zeros(shape, dtype=np.int8)
+    for d in range(D):
+        if t == 0 or (S[d] == 1 and per[d]):
+            continue
+        M = shape[d] // S[d]
+        e = np.arange(shape[d]) % M
+        is_edge = ((e < t) | (e >= M - t)).astype(np.int8)
+        sh = [1] * D
+        sh[d] = shape[d]
+        count = count + is_edge.reshape(sh)
+    return count >= 1, count >= 2
+
+
+def check_field(got, ref, tol, shape, S, t, periodic=None, what=""):
+    """The bar of BASELINE.json (relative L2 <= tol over the grid) plus a per-voxel bar on the voxels the
+    slab logic touches: there the largest absolute error must stay within 2 x tol x max|ref| (about 10 x tol x rms
+    for white noise; fp32 FFT rounding scales with the largest magnitudes on a line, not with the local value, so a
+    field concentrated around a point source is measured against its peak).  A handful of wrong slab voxels can hide
+    under an L2 norm over the grid; they cannot hide here (an unapplied or misplaced correction is O(0.1..1) x the
+    local values)."""
+    got = np.asarray(got).astype(np.complex128)
+    ref = np.asarray(ref).astype(np.complex128)
+    r = rel(got, ref)
+    assert r <= tol, (what, "rel-L2", r)
+    slab, multi = edge_masks(shape, S, t, periodic)
+    peak = float(np.abs(ref).max())
+    err = np.abs(got - ref)
+    for name, mask in (("slab voxels", slab), ("multi-axis edge voxels", multi)):
+        if mask.any():
+            worst = float(err[mask].max())
+            assert worst <= 2.0 * tol * peak, (what, name, worst, peak)
+    return r
+
+
+_CASE_CACHE = {}
+
+
+def cached(key, fn):
+    """Oracle results are the same for every kernel variant of a case: compute them once per session."""
+    if key not in _CASE_CACHE:
+        _CASE_CACHE[key] = fn()
+    return _CASE_CACHE[key]
+
+
 def make_pair(B, orc, shape, S, W, t, periodic=None, seed=0, medium=None):
     n = medium if medium is not None else workloads.random_medium(shape, 100 + seed, 1.0, 1.5, 0.02)
     o = orc.MBSOracle(n, 0.25, 1.0, W, S, periodic=periodic, n_correction=t)
@@ -57,6 +109,37 @@ OPERATOR_CASES = [
     ((16, 32, 128), (2, 2, 2), (2, 2, 2), 4, (1, 0, 0)),
 ]
 
+# The FFT plans the BASELINE.json configs instantiate, each subdomain length in each role it plays there
+# (VERDICT r01 "what's weak" 1): 256 and 512 (cfg 2, 3, 5), 320 (cfg 4), plus 160 and 384, as
+#   contiguous axis (warp-line first / last sweep, T = 32 lanes per line for 512),
+#   axis-1 strided forward / inverse sweep (TMA boxes; 512 rows = two boxes), ragged inner tail,
+#   axis-0 kernel-multiply sweep in 3-D and 2-D (|p|^2 table per inner index).
+PLAN_CASES = [
+    ((16, 16, 256), (1, 1, 1), (2, 2, 8), 8, None),          # 256 contiguous
+    ((16, 16, 512), (1, 1, 2), (2, 2, 8), 8, None),          # 256 contiguous, two subdomains along the line
+    ((16, 16, 512), (1, 1, 1), (2, 2, 8), 8, None),          # 512 contiguous
+    ((16, 16, 1024), (1, 1, 2), (2, 2, 8), 8, None),         # 512 contiguous, two subdomains along the line
+    ((16, 256, 40), (1, 1, 1), (2, 8, 4), 8, None),          # 256 strided on axis 1, inner 40 = 32 + ragged 8
+    ((16, 512, 40), (1, 1, 1), (2, 8, 4), 8, None),          # 512 strided on axis 1 (two TMA boxes), ragged tail
+    ((16, 1024, 40), (1, 2, 1), (2, 8, 4), 8, None),         # 512 strided on axis 1, two subdomains
+    ((256, 16, 40), (1, 1, 1), (8, 2, 4), 8, None),          # 256 kernel-multiply sweep on axis 0, 3-D
+    ((512, 16, 40), (1, 1, 1), (8, 2, 4), 8, None),          # 512 kernel-multiply sweep on axis 0, 3-D
+    ((1024, 16, 40), (4, 1, 1), (8, 2, 4), 8, None),         # 256 on axis 0, four subdomains (cfg 5 layout)
+    ((256, 40), (1, 1), (8, 4), 8, None),                    # 256 kernel-multiply sweep, 2-D
+    ((1024, 40), (2, 1), (8, 4), 8, None),                   # 512 kernel-multiply sweep, 2-D, two subdomains (cfg 2)
+    ((640, 16, 16), (2, 1, 1), (8, 2, 2), 8, None),          # 320 on axis 0 (cfg 4)
+    ((16, 320, 40), (1, 1, 1), (2, 8, 4), 8, None),          # 320 strided on axis 1 (two-CTA, two-stage path)
+    ((16, 640, 40), (1, 2, 1), (2, 8, 4), 8, None),          # 320 strided on axis 1, two subdomains
+    ((160, 40), (1, 1), (8, 4), 8, None),                    # 160
+    ((16, 160, 40), (1, 1, 1), (2, 8, 4), 8, None),
+    ((16, 16, 320), (1, 1, 2), (2, 2, 8), 8, None),          # 160 contiguous
+    ((384, 40), (1, 1), (8, 4), 8, None),                    # 384
+    ((16, 384, 40), (1, 1, 1), (2, 8, 4), 8, None),
+    ((16, 16, 384), (1, 1, 1), (2, 2, 8), 8, None),
+    ((128, 256, 32), (1, 1, 1), (4, 4, 4), 8, None),         # cfg 3's subdomain lengths on axes 0, 1
+]
+OPERATOR_CASES = OPERATOR_CASES + PLAN_CASES
+
 
 @pytest.mark.parametrize("shape,S,W,t,periodic", OPERATOR_CASES)
 def test_operator_parity(B, orc, shape, S, W, t, periodic):
@@ -78,12 +161,12 @@ def test_operator_parity(B, orc, shape, S, W, t, periodic):
     }
     for which, ref in refs.items():
         got = s.apply_operator(which, u).cpu().numpy()
-        assert rel(got, ref) <= OP_TOL, (which, rel(got, ref))
+        check_field(got, ref, OP_TOL, shape, S, t, periodic, what=which)
     # in == out is allowed
     import torch
     ud = torch.from_numpy(u).cuda()
     s.apply_operator(B.MBS_OP_PRECOND_A, ud, out=ud)
-    assert rel(ud.cpu().numpy(), refs[B.MBS_OP_PRECOND_A]) <= OP_TOL
+    check_field(ud.cpu().numpy(), refs[B.MBS_OP_PRECOND_A], OP_TOL, shape, S, t, periodic, what="in == out")
     s.close()
 
 
@@ -116,12 +199,12 @@ def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line, me
     y = workloads.random_field(shape, 21)
     x0 = workloads.random_field(shape, 22)
     n_it = 6
-    x_ref, h_ref = o.solve(y, x0=x0, tol=0.0, max_iter=n_it)
+    x_ref, h_ref = cached(("iter", shape, S, W, t, periodic), lambda: o.solve(y, x0=x0, tol=0.0, max_iter=n_it))
     yd = torch.from_numpy(y).cuda()
     xd = torch.from_numpy(x0).cuda()
     hist = s.iterate(yd, xd, n_it)
     assert np.allclose(hist, h_ref, rtol=2e-5), (hist, h_ref)
-    assert rel(xd.cpu().numpy(), x_ref) <= OP_TOL, rel(xd.cpu().numpy(), x_ref)
+    check_field(xd.cpu().numpy(), x_ref, OP_TOL, shape, S, t, periodic, what="iterate")
     # the same through mbs_solve (stop flag path): identical history, bit for bit
     x2, hist2, rc = s.solve(y, x0=x0, tol=0.0, max_iter=n_it)
     assert rc == B.MBS_ERR_NOT_CONVERGED
@@ -204,7 +287,7 @@ def test_solve_parity(B, orc, name, make, fused):
         assert rc == B.MBS_OK
         slack = count_slack(h_ref, w.tol, floor)
         assert abs(len(hist) - len(h_ref)) <= slack, (len(hist), len(h_ref), slack, floor)
-        err = rel(x.cpu().numpy(), x_ref)
+        err = check_field(x.cpu().numpy(), x_ref, FIELD_TOL, w.shape, w.n_subdomains, w.n_correction, what=name)
         print("%s: floor %.2e tol %.1e iterations %d (oracle %d, slack %d) field rel-L2 %.2e"
               % (name, floor, w.tol, len(hist), len(h_ref), slack, err))
         assert err <= FIELD_TOL, err
@@ -216,7 +299,7 @@ def test_solve_parity(B, orc, name, make, fused):
         x, hist, rc = s.solve(y, tol=thr, max_iter=w.max_iter)
         x_ref2, h_ref2 = o.solve(y, tol=thr, max_iter=w.max_iter)
         assert rc == B.MBS_OK and abs(len(hist) - len(h_ref2)) <= 1
-        err = rel(x.cpu().numpy(), x_ref2)
+        err = check_field(x.cpu().numpy(), x_ref2, FIELD_TOL, w.shape, w.n_subdomains, w.n_correction, what=name)
         print("%s: floor %.2e >= 0.7 tol %.1e; compared at %.2e: iterations %d (oracle %d) field rel-L2 %.2e"
               % (name, floor, w.tol, thr, len(hist), len(h_ref2), err))
         assert err <= FIELD_TOL, err
@@ -308,6 +391,13 @@ def test_non_finite_residual_is_reported(B):
     with pytest.raises(B.MBSError) as e:
         s.solve(y, x0=x0, tol=1e-3, max_iter=200)
     assert e.value.status == B.MBS_ERR_NUMERIC
+    # a NaN (or Inf) in the refractive-index map is refused at mbs_set_potential, not discovered later in a solve
+    for bad in (np.nan, np.inf, complex(1.2, np.nan)):
+        n_bad = w.make_medium()
+        n_bad[5, 6, 7] = bad
+        with pytest.raises(B.MBSError) as e:
+            s.set_potential(n_bad)
+        assert e.value.status == B.MBS_ERR_NUMERIC, bad
     s.close()
 
 
@@ -388,15 +478,24 @@ def test_full_size_properties_cfg5(B):
 
 
 MID_SIZE_CASES = [
-    ("cfg4_160", lambda: workloads.config(4, shape=(160, 160, 160), boundary_width=(12, 12, 12))),
-    ("cfg5_256", lambda: workloads.config(5, shape=(256, 256, 256), boundary_width=(16, 16, 16))),
+    # name, workload, number of updates compared
+    ("cfg4_160", lambda: workloads.config(4, shape=(160, 160, 160), boundary_width=(12, 12, 12)), 10),
+    ("cfg5_256", lambda: workloads.config(5, shape=(256, 256, 256), boundary_width=(16, 16, 16)), 10),
+    # FULL-SIZE configs 2 and 3 of BASELINE.json: 512-long lines on both axes of cfg 2,
+    # 128 x 256 x 256 subdomains of cfg 3, in the launch configuration bench.py times
+    ("cfg2_full", lambda: workloads.config(2), 10),
+    ("cfg3_full", lambda: workloads.config(3), 10),
+    # one subdomain of config 5 in its real aspect (256 x 512 x 512: Plan<256> on axis 0, Plan<512> on axes 1 and 2,
+    # two TMA boxes per tile, T = 32 lanes per line, 2^18 entries in the per-line |p|^2 table)
+    ("cfg5_one_subdomain", lambda: dataclasses.replace(
+        workloads.config(5, shape=(256, 512, 512), boundary_width=(16, 16, 16)), n_subdomains=(1, 1, 1)), 3),
 ]
 
 
-@pytest.mark.parametrize("name,make", MID_SIZE_CASES)
-def test_operators_and_first_residuals_mid_size(B, orc, name, make):
-    """Parity plan of SURVEY 8(d) for configs 4-5 at the largest size the oracle handles in about a minute (same
-    generators and subdomain counts): (i) per-operator parity on a seeded random vector, (ii) the first 10 residuals."""
+@pytest.mark.parametrize("name,make,n_it", MID_SIZE_CASES)
+def test_operators_and_first_residuals_mid_size(B, orc, name, make, n_it):
+    """Parity plan of SURVEY 8(d) at the sizes the oracle handles in about a minute (same generators): (i) per-operator
+    parity on a seeded random vector, (ii) the first residuals and the iterate after them."""
     import torch
     w = make()
     n, y = w.make_medium(), w.make_source()
@@ -405,16 +504,109 @@ def test_operators_and_first_residuals_mid_size(B, orc, name, make):
     s.set_potential(n)
     u = workloads.random_field(w.shape, 31)
     u128 = u.astype(np.complex128)
-    for which, ref in ((B.MBS_OP_B, o.apply_B(u128)), (B.MBS_OP_PROPAGATOR, o.propagate(u128)),
-                       (B.MBS_OP_PRECOND_A, o.apply_precond_A(u128))):
+    geom = (w.shape, w.n_subdomains, w.n_correction)
+    for which, fn in ((B.MBS_OP_B, o.apply_B), (B.MBS_OP_PROPAGATOR, o.propagate), (B.MBS_OP_PRECOND_A, o.apply_precond_A)):
+        ref = fn(u128)
         got = s.apply_operator(which, u).cpu().numpy()
-        assert rel(got, ref) <= OP_TOL, (which, rel(got, ref))
-    x_ref, h_ref = o.solve(y, tol=0.0, max_iter=10)
+        check_field(got, ref, OP_TOL, *geom, what=(name, which))
+        del ref, got
+    x_ref, h_ref = o.solve(y, tol=0.0, max_iter=n_it)
     yd = torch.from_numpy(y).cuda()
     xd = torch.zeros(w.shape, dtype=torch.complex64, device="cuda")
-    hist = s.iterate(yd, xd, 10)
+    hist = s.iterate(yd, xd, n_it)
     assert np.allclose(hist, h_ref, rtol=1e-4), (hist, h_ref)
-    assert rel(xd.cpu().numpy(), x_ref) <= OP_TOL
+    check_field(xd.cpu().numpy(), x_ref, OP_TOL, *geom, what=(name, "iterate"))
+    s.close()
+
+
+def _host_ram_gib():
+    import psutil
+    return psutil.virtual_memory().available / 2 ** 30
+
+
+@pytest.mark.slow
+def test_full_size_cfg5_operators_vs_oracle(B, orc):
+    """Config 5 at FULL size (1024^3, 4x2x2 subdomains, the launch configuration bench.py times): B, (L+I)^-1 and
+    Gamma^-1 A on a seeded random vector against the oracle, voxel by voxel (SURVEY 8(d) parity plan (i)), and the first
+    three residuals (plan (ii)).  The complex128 oracle needs about 120 GiB of host memory and 10-20 minutes at this
+    size, so the test is opt-in (`--run-slow`); its printed result is recorded in profiles/."""
+    import torch
+    if torch.cuda.mem_get_info()[0] < 90 * 2 ** 30:
+        pytest.skip("needs about 80 GiB of free device memory")
+    if _host_ram_gib() < 150:
+        pytest.skip("the complex128 oracle at 1024^3 needs about 120 GiB of host memory (%.0f GiB available)" % _host_ram_gib())
+    w = workloads.config(5)
+    n, y = w.make_medium(), w.make_source()
+    s = B.Solver.from_workload(w)
+    s.set_potential(torch.from_numpy(n).cuda())
+    o = orc.from_workload(w, n)
+    del n
+    info = s.info()
+    assert info["c"] == pytest.approx(o.c, rel=1e-12) and info["k02"] == pytest.approx(o.k02, rel=1e-12)
+    u = workloads.random_field(w.shape, 31)
+    ud = torch.from_numpy(u).cuda()
+    slab, multi = edge_masks(w.shape, w.n_subdomains, w.n_correction)
+
+    def compare(got_dev, ref, what):
+        got = got_dev.cpu().numpy()
+        num = den = 0.0
+        worst_slab = worst_multi = peak = 0.0
+        for i0 in range(0, w.shape[0], 64):                     # chunked: no second 16 GiB temporary
+            sl = slice(i0, i0 + 64)
+            e = np.abs(got[sl] - ref[sl])
+            num += float(np.sum(e * e))
+            den += float(np.sum(np.abs(ref[sl]) ** 2))
+            worst_slab = max(worst_slab, float(e[slab[sl]].max()))
+            worst_multi = max(worst_multi, float(e[multi[sl]].max()))
+            peak = max(peak, float(np.abs(ref[sl]).max()))
+        r = np.sqrt(num / den)
+        print("cfg5 full size %s: rel-L2 %.2e, worst slab voxel %.2e x peak, worst multi-axis edge voxel %.2e x peak"
+              % (what, r, worst_slab / peak, worst_multi / peak))
+        assert r <= OP_TOL and worst_slab <= 2 * OP_TOL * peak and worst_multi <= 2 * OP_TOL * peak
+
+    u128 = u.astype(np.complex128)
+    del u
+    compare(s.apply_operator(B.MBS_OP_B, ud), o.apply_B(u128), "B")
+    compare(s.apply_operator(B.MBS_OP_PROPAGATOR, ud), o.propagate(u128), "(L+I)^-1")
+    compare(s.apply_operator(B.MBS_OP_PRECOND_A, ud), o.apply_precond_A(u128), "Gamma^-1 A")
+    del u128, ud
+    x_ref, h_ref = o.solve(y, tol=0.0, max_iter=3)
+    yd = torch.from_numpy(y).cuda()
+    xd = torch.zeros(w.shape, dtype=torch.complex64, device="cuda")
+    hist = s.iterate(yd, xd, 3)
+    print("cfg5 full size residuals: gpu %s oracle %s" % (hist, h_ref))
+    assert np.allclose(hist, h_ref, rtol=1e-4), (hist, h_ref)
+    compare(xd, x_ref, "x after 3 updates")
+    s.close()
+
+
+FULL_SOLVE_CASES = [("cfg2_full", lambda: workloads.config(2)), ("cfg3_full", lambda: workloads.config(3))]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("name,make", FULL_SOLVE_CASES)
+def test_full_size_converged_field_vs_oracle(B, orc, name, make):
+    """Configs 2 and 3 of BASELINE.json at FULL size, solved to their own tol on both sides: converged field <= 1e-4,
+    iteration counts within the floor-derived slack of DESIGN.md section 7 (BASELINE.md section 3 plan).  The oracle
+    solve takes tens of minutes (cfg 2: ~1.6e4 iterations of a 1024^2 grid; cfg 3: ~1.7e3 of 256^3), so the test is
+    opt-in (`--run-slow`); its printed result is recorded in profiles/."""
+    w = make()
+    n, y = w.make_medium(), w.make_source()
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    x, hist, rc = s.solve(y, tol=w.tol, max_iter=w.max_iter)
+    nu = s.info()["norm_rhs"]
+    xc = x.clone()
+    import torch
+    floor = min(float(hist.min()), float(s.iterate(torch.from_numpy(y).cuda(), xc, 2000, nu=nu).min()))
+    o = orc.from_workload(w, n)
+    x_ref, h_ref = o.solve(y, tol=w.tol, max_iter=w.max_iter)
+    slack = count_slack(h_ref, w.tol, floor)
+    err = check_field(x.cpu().numpy(), x_ref, FIELD_TOL, w.shape, w.n_subdomains, w.n_correction, what=name)
+    print("%s FULL SIZE: status %s, floor %.2e, tol %.1e, iterations %d (oracle %d, slack %d), field rel-L2 %.2e"
+          % (name, B.STATUS_NAMES[rc], floor, w.tol, len(hist), len(h_ref), slack, err))
+    assert rc == B.MBS_OK
+    assert abs(len(hist) - len(h_ref)) <= slack
     s.close()
 
 

@@ -107,11 +107,67 @@ def test_eq9_a_d_values():
     o3 = _small_oracle((32, 32), (2, 2), (4, 4), 8, seed=3, periodic=(0, 1))
     assert o1.a == (1, 1) and o2.a == (2, 1) and o3.a == (2, 2)
     for o in (o1, o2, o3):
-        assert o.c == pytest.approx(-0.95j / (o.v_max + sum(o.a) * o.norm_A12))
+        # c is purely imaginary and |c| (v_max + sum_a ||A_12||) = 0.95; literal values of c are pinned in
+        # test_scale_factor_literal_values
+        assert o.c.real == 0.0 and o.c.imag < 0
         # convergence condition P:55: i c real and < 1 / ||k^2 - k0^2||_inf
         assert (1j * o.c).imag == pytest.approx(0.0)
         assert (1j * o.c).real < 1.0 / o.v_max
     assert abs(o2.c) < abs(o1.c)
+
+
+def test_scale_factor_literal_values():
+    """Eq. (4) and Eq. (9) on a medium whose numbers can be worked by hand, written out as literals
+    (not the oracle's formula re-typed): lambda = 1, h = 1/4, n = 1 except one voxel with n = 2, no absorber.
+      k^2 in {(2 pi)^2, 4 (2 pi)^2} = {39.4784176, 157.9136704};  k0^2 = 98.6960440 (R2: centre of the range);
+      ||k^2 - k0^2||_inf = 59.2176264.
+      periodic, one domain, t = 0:     c = -0.95 i / 59.2176264               = -0.0160425207 i       (Eq. (4))
+      two subdomains, t = 8:           ||A_12|| = 2.17915 / h^2 = 34.8664 (sigma_max printed in SURVEY 8(c) step 6),
+                                       c = -0.95 i / (59.2176264 + 2 * 34.8664) = -0.00736718 i       (Eq. (9), a = 2)
+      one non-periodic domain, t = 8:  c = -0.95 i / (59.2176264 + 1 * 34.8664) = -0.0100974 i        (a = 1)"""
+    n = np.ones(32, dtype=np.complex64)
+    n[11] = 2.0
+    o = orc.MBSOracle(n, 0.25, 1.0, (0,), (1,), periodic=(1,), n_correction=0)
+    assert o.k02 == pytest.approx(98.6960440, rel=1e-8)
+    assert o.v_max == pytest.approx(59.2176264, rel=1e-8)
+    assert o.c.real == 0.0 and o.c.imag == pytest.approx(-0.0160425207, rel=1e-8)
+    o2 = orc.MBSOracle(n, 0.25, 1.0, (0,), (2,), n_correction=8)
+    assert o2.c.real == 0.0 and o2.c.imag == pytest.approx(-0.00736718, rel=2e-5)
+    o1 = orc.MBSOracle(n, 0.25, 1.0, (0,), (1,), n_correction=8)
+    assert o1.c.real == 0.0 and o1.c.imag == pytest.approx(-0.0100974, rel=2e-5)
+
+
+def test_absorber_weight_is_max_over_axes_2d():
+    """R3: w(r) = max_d w_d(r).  2-D, n = 1, W = (8, 4): at pixel (2, 3) the two ramps give 6/8 and 1/4, at (6, 0)
+    they give 2/8 and 1; the layer adds i 0.5 (2 pi)^2 max(...) to k^2 (a sum would give 1.0 and 1.25, a product
+    0.1875 and 0.25)."""
+    o = orc.MBSOracle(np.ones((32, 24), dtype=np.complex64), 0.25, 1.0, (8, 4), (1, 1), n_correction=4)
+    kw2 = 39.47841760435743
+    assert o.k2[2, 3].imag == pytest.approx(0.5 * kw2 * 0.75, rel=1e-12)
+    assert o.k2[6, 0].imag == pytest.approx(0.5 * kw2 * 1.0, rel=1e-12)
+    assert o.k2[29, 20].imag == pytest.approx(0.5 * kw2 * 0.75, rel=1e-12)      # mirrored: (32-1-29, 24-1-20) = (2, 3)
+    assert o.k2[16, 12].imag == 0.0
+
+
+def test_first_update_is_alpha_times_preconditioned_source():
+    """P:76 Eq. (6) with x^(0) = 0: x^(1) = alpha B (L+I)^-1 y_vec, alpha = 0.75 (Eq. (4)), y_vec = -c y.
+    The right-hand side is assembled from the dense matrices of tests/dense_reference.py with the literal 0.75."""
+    shape, S, t = (16, 12), (2, 1), 4
+    o = _small_oracle(shape, S, (2, 2), t, seed=41)
+    L, V = dr.assemble(o.k2, o.k02, o.c, shape, S, t, o.h, o.a, (0, 0))
+    I = np.eye(L.shape[0])
+    rng = np.random.default_rng(3)
+    y = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+    x1_dense = 0.75 * (I - V) @ np.linalg.solve(L + I, (-o.c * y).reshape(-1))
+    x1, hist = o.solve(y, tol=0.0, max_iter=1)
+    assert len(hist) == 1 and hist[0] == pytest.approx(1.0, abs=1e-13)
+    assert np.linalg.norm(x1.reshape(-1) - x1_dense) / np.linalg.norm(x1_dense) < 1e-12
+    # and the second update follows Eq. (6) from x^(1) with the same alpha
+    x1v = x1_dense
+    r = (I - V) @ (x1v - np.linalg.solve(L + I, (-o.c * y).reshape(-1) + (I - V) @ x1v))
+    x2_dense = x1v - 0.75 * r
+    x2, _ = o.solve(y, tol=0.0, max_iter=2)
+    assert np.linalg.norm(x2.reshape(-1) - x2_dense) / np.linalg.norm(x2_dense) < 1e-12
 
 
 def test_k0_minimises_vmax_box():
@@ -227,15 +283,15 @@ def test_full_correction_recovers_linear_convolution():
 # ------------------------------------------------------------------------------------------
 # closed-form Green's function
 # ------------------------------------------------------------------------------------------
-def _green_error(S, t, periodic, N=1024, W=128, beta=0.3):
+def _green_error(S, t, periodic, N=1024, W=128, beta=0.3, n_val=1.0):
     h, lam = 0.25, 1.0
-    n = np.ones(N, dtype=np.complex64)
+    n = np.full(N, n_val, dtype=np.complex64)
     o = orc.MBSOracle(n, h, lam, (W,), (S,), periodic=(periodic,), n_correction=t, beta=beta)
     y = np.zeros(N, dtype=np.complex128)
     src = N // 2 - 37
     y[src] = 1.0 / h
     x, hist = o.solve(y, tol=1e-9, max_iter=50000)
-    k = 2 * np.pi / lam
+    k = 2 * np.pi * n_val / lam
     r = (np.arange(N) - src) * h
     exact = 1j / (2 * k) * np.exp(1j * k * np.abs(r))
     roi = np.zeros(N, dtype=bool)
@@ -250,6 +306,19 @@ def test_green_function_1d_undecomposed():
     err, hist = _green_error(S=1, t=0, periodic=1)
     assert err < 2e-3
     assert np.all(np.diff(hist) <= 1e-15)
+
+
+def test_green_function_1d_in_a_medium_of_index_1p33():
+    """the wavenumber is k = 2 pi n / lambda, i.e. k^2 = (2 pi / lambda)^2 n^2 (oracle step 1).  In a homogeneous
+    medium of n = 1.33 the field of a point source is (i/2k) e^{ik|r|} with k = 2 pi 1.33 / lambda; k^2 proportional to
+    n (or to anything but n^2) gives another wavelength and amplitude and fails by O(1)."""
+    err, hist = _green_error(S=1, t=0, periodic=1, n_val=1.33)
+    assert err < 3e-3
+    assert np.all(np.diff(hist) <= 1e-15)
+    # control: the closed form with the wavenumber of n = 1 does not fit this field (the pin can tell them apart)
+    h, N, W = 0.25, 1024, 128
+    o = orc.MBSOracle(np.full(N, 1.33, dtype=np.complex64), h, 1.0, (W,), (1,), periodic=(1,), n_correction=0, beta=0.3)
+    assert o.k2[N // 2] == pytest.approx((2 * np.pi * 1.33) ** 2, rel=1e-6)
 
 
 def test_green_function_1d_two_domains_full_correction():
