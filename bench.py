@@ -2,6 +2,7 @@
 """bench.py -- throughput of the fused MBS iteration (BASELINE.json metric) on N B200s of one node.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3|4|5] [--impl b200|reference]
+    python bench.py --converge-config 3|4|5      (cold-start solve to the config's tol: seconds and iterations)
 
 A "step" is one iteration of Eq. (6) of the paper over the whole grid: every row of
 SURVEY.md 8(a) (scattering operator with edge-slab corrections, per-subdomain FFT propagator, difference,
@@ -12,7 +13,9 @@ Output: ONE JSON line (rank 0).  `value` = voxel-iterations/s with every input r
 events on the solver's stream, max over ranks; `e2e` = the same metric through the host-buffer entry point
 mbs_solve_host (H2D of y and x0 and D2H of x inside the timed region); `roofline` = the dominant kernel's
 algorithmic bytes per launch / its average event-timed duration against MEASURED_PEAKS.json; `cpu_baseline` =
-the CPU oracle, as it stands, timed on a bounded sample on this box's host cores.
+the CPU oracle, as it stands, timed on a bounded sample on this box's host cores.  The default run (no --config)
+times the two other 3-D configs of BASELINE.json as well (same K-step event timing) and reports them under
+`other_configs`, each against the 112 B floor ledger and against its own sparse-source ledger.
 
 Multi-GPU: the path does not shard in this build (BASELINE.json: "no sharding, no collectives"): --gpus N runs N
 independent replicas ("replicas only"); value = N x voxels x K / max-over-ranks time.
@@ -37,7 +40,14 @@ import numpy as np
 
 METRIC = "Gvoxel-iterations/s of fused MBS step"
 UNIT = "Gvoxel-it/s"
-SAMPLE_SHAPES = {3: (128, 128, 128), 4: (160, 160, 160), 5: (256, 128, 128)}   # oracle sample grids
+# Oracle samples (cpu_baseline, --impl reference): config 3 itself; for configs 4 and 5 ONE subdomain of the workload in
+# its real shape (same generator; the per-subdomain FFTs, the largest part of an oracle iteration, are exactly those of the
+# full grid).  The full grids need 30 / 120 GiB of complex128 arrays and minutes per oracle iteration, outside the
+# 10-30 s budget of this leg; `--cpu-baseline-full` times the oracle on the workload itself when the host has the memory.
+SAMPLE_GRIDS = {3: ((256, 256, 256), (2, 1, 1), (16, 16, 16)),
+                4: ((320, 320, 320), (1, 1, 1), (24, 24, 24)),
+                5: ((256, 512, 512), (1, 1, 1), (32, 32, 32))}
+DEFAULT_STEPS = {3: 400, 4: 60, 5: 30}
 
 
 def parse_args():
@@ -45,12 +55,18 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
-    ap.add_argument("--config", type=int, default=5, choices=(3, 4, 5))
+    ap.add_argument("--config", type=int, default=None, choices=(3, 4, 5),
+                    help="workload (default 5; without this flag configs 3 and 4 are timed too, under other_configs)")
+    ap.add_argument("--converge-config", type=int, default=None, choices=(3, 4, 5),
+                    help="only: cold-start mbs_solve of this config at its tol; prints seconds and iterations")
+    ap.add_argument("--cpu-baseline-full", action="store_true",
+                    help="time the oracle on the workload itself (3 iterations; config 5 needs ~120 GiB of host memory)")
     ap.add_argument("--impl", default="b200", choices=("b200", "reference"))
     ap.add_argument("--shape", default=None, help="override the grid, e.g. 256,512,1024 (profiling runs; not the headline)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-converge", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true", help="default run: do not time configs 3 and 4 as well")
     ap.add_argument("--unfused", action="store_true", help="one kernel per step of P:122-128 instead of the fused sweeps")
     return ap.parse_args()
 
@@ -101,13 +117,21 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_sample(cfg, n_iter, budget_s=25.0, warmup=1):
-    """Time the CPU oracle (oracle/mbs_oracle.py, as it stands) on a bounded sample of config `cfg`: the same
-    generator and subdomain counts at a reduced grid, `n_iter` iterations of Eq. (6).  Returns a dict."""
+def oracle_sample(cfg, n_iter, budget_s=25.0, warmup=1, full=False):
+    """Time the CPU oracle (oracle/mbs_oracle.py, as it stands) on a bounded sample of config `cfg` (SAMPLE_GRIDS), or on
+    the workload itself (`full`), `n_iter` iterations of Eq. (6) at most `budget_s` seconds.  Returns a dict."""
+    import dataclasses
     from paper_2410_02395_b200 import workloads
     from oracle import mbs_oracle
-    shape = SAMPLE_SHAPES[cfg]
-    w = workloads.config(cfg, shape=shape, boundary_width=(8, 8, 8))
+    if full:
+        w = workloads.config(cfg)
+        what = "the workload itself"
+    else:
+        shape, S, W = SAMPLE_GRIDS[cfg]
+        w = dataclasses.replace(workloads.config(cfg, shape=shape, boundary_width=W), n_subdomains=S)
+        what = ("the workload itself" if shape == workloads.config(cfg).shape else
+                "one subdomain of the workload in its real shape (the full grid needs %d GiB of complex128 arrays and minutes "
+                "per oracle iteration: outside this leg's budget)" % (workloads.config(cfg).voxels * 16 * 7 // 2 ** 30))
     n, y = w.make_medium(), w.make_source()
     o = mbs_oracle.from_workload(w, n)
     times = []
@@ -129,8 +153,8 @@ def oracle_sample(cfg, n_iter, budget_s=25.0, warmup=1):
     steady = times[warmup:] if len(times) > warmup else times[-1:]
     per_it = float(np.mean(steady))
     return {"value": w.voxels / per_it / 1e9, "unit": UNIT, "cores": mbs_oracle._workers(), "kind": "oracle",
-            "sample": "cfg%d generator at %s with %s subdomains, %d oracle iterations (numpy complex128, scipy.fft)"
-                      % (cfg, "x".join(map(str, shape)), "x".join(map(str, w.n_subdomains)), len(steady)),
+            "sample": "cfg%d generator at %s with %s subdomains = %s; %d oracle iteration(s) timed (numpy complex128, scipy.fft)"
+                      % (cfg, "x".join(map(str, w.shape)), "x".join(map(str, w.n_subdomains)), what, len(steady)),
             "ms_per_step": per_it * 1e3, "voxels": w.voxels}
 
 
@@ -139,19 +163,28 @@ def _workloads():
     return workloads
 
 
+def config_block(w, world):
+    """The `config` object of the JSON line: the same on both arms (the driver compares them)."""
+    return {"workload": workload_name(w),
+            "l2": "inputs larger than L2 (%.1f GiB per array): no flush between iterations" % (w.voxels * 8 / 2 ** 30)
+                  if w.voxels * 8 > 4 * 126e6 else "arrays comparable to L2; no flush (the step streams 4 arrays)",
+            "parallelism": "replicas x%d (the path does not shard in this build)" % world}
+
+
 def run_reference(args):
-    """--impl reference: the oracle is the only reference implementation of this paper available here."""
+    """--impl reference: the oracle is the only reference implementation of this paper available here.  A step is one
+    oracle iteration on the bounded sample of the workload (SAMPLE_GRIDS); the run stops early after 4 minutes."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
+    cfg = args.config or 5
     K = args.steps if args.steps is not None else 5
     W = args.warmup if args.warmup is not None else 1
-    r = oracle_sample(args.config, K + W, budget_s=120.0, warmup=W)
+    r = oracle_sample(cfg, K + W, budget_s=240.0, warmup=W, full=args.cpu_baseline_full)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": K,
             "warmup": W, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "c128", "data": "synthetic",
-            "config": {"workload": workload_name(_workloads().config(args.config)),
-                       "sample": r["sample"]},
+            "config": config_block(_workloads().config(cfg), max(1, args.gpus)),
             "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -164,10 +197,14 @@ def workload_name(w):
         "x".join(map(str, w.boundary_width)))
 
 
+TRAFFIC_SOURCE = ("dram__bytes_read.sum + dram__bytes_write.sum per voxel from the committed ncu --set full capture "
+                  "(profiles/dram_traffic.json, measured on a smaller grid with the same line lengths), scaled to this "
+                  "workload's voxel count; not measured in this run")
+
+
 def dominant_kernel_traffic(name, voxels):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of kernel class `name`: measured per voxel in the committed
-    ncu --set full capture (profiles/dram_traffic.json, from profiles/r01_ncu_full_summary.md, a smaller grid of the same
-    line lengths) and scaled to this workload's voxel count.  None when the kernel is not in the capture."""
+    """DRAM bytes per launch of kernel class `name`, scaled from profiles/dram_traffic.json (see TRAFFIC_SOURCE).
+    None when the kernel is not in the capture."""
     path = os.path.join(ROOT, "profiles", "dram_traffic.json")
     if not os.path.exists(path):
         return None
@@ -194,33 +231,23 @@ def aggregate_throughput(voxels, steps, ms, world):
     return world * voxels * steps / (ms * 1e-3) / 1e9
 
 
-def run_b200(args):
+def time_config(cfg, K, W, dev, world, shape=None, unfused=False, options=()):
+    """K timed iterations of Eq. (6) on BASELINE.json config `cfg` after W warm-up iterations, everything resident in
+    HBM, CUDA events on the solver's stream, max over ranks.  Returns (solver, workload, y_dev, x_dev, result dict)."""
     import torch
     import torch.distributed as dist
     from paper_2410_02395_b200 import binding, workloads
-
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    K = args.steps if args.steps is not None else {3: 400, 4: 60, 5: 30}[args.config]
-    W = args.warmup if args.warmup is not None else 3
-    W = max(W, 3)
-
-    w = workloads.config(args.config, shape=tuple(int(v) for v in args.shape.split(",")) if args.shape else None)
+    w = workloads.config(cfg, shape=shape)
     t0 = time.perf_counter()
     n_map, y = w.make_medium(), w.make_source()
     t_gen = time.perf_counter() - t0
     s = binding.Solver.from_workload(w, device=dev)
-    s.set_option(binding.MBS_OPT_FUSED, 0 if args.unfused else 1)
+    s.set_option(binding.MBS_OPT_FUSED, 0 if unfused else 1)
+    for opt, val in options:
+        s.set_option(opt, val)
     nd = torch.from_numpy(n_map).to(dev)
     s.set_potential(nd)
-    del nd
+    del nd, n_map
     yd = torch.from_numpy(y).to(dev)
     xd = torch.zeros(w.shape, dtype=torch.complex64, device=dev)
     torch.cuda.synchronize()
@@ -243,7 +270,7 @@ def run_b200(args):
 
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
-    with ClockSampler(local) as clocks:
+    with ClockSampler(dev.index) as clocks:
         ev0.record(s.stream)
         hist = s.iterate(yd, xd, K, nu=nu)
         ev1.record(s.stream)
@@ -259,40 +286,51 @@ def run_b200(args):
     ms = max_over_ranks(ms, dev)
     value = aggregate_throughput(w.voxels, K, ms, world)
 
-    # roofline of the dominant kernel
     peak, peak_kind = peaks()
     stats = [k for k in stats if k["launches"] > 0]
     stats.sort(key=lambda k: -k["total_ms"])
-    total_kernel_ms = sum(k["total_ms"] for k in stats)
+    info = s.info()
+    floor_bytes = info["algorithmic_bytes_per_iteration"]            # 112 B/voxel in 3-D: the quoted denominator
+    sparse_bytes = info["sparse_source_bytes_per_iteration"]          # minus the all-zero rows of y this workload skips
+    per_s = K / (ms * 1e-3) / 1e9 * world
+    kernels = [{"name": k["name"], "launches_per_step": k["launches"] / K, "avg_ms": k["total_ms"] / k["launches"],
+                "GBps": k["algorithmic_bytes"] / max(k["total_ms"], 1e-9) / 1e6} for k in stats]
+    res = {"cfg": cfg, "workload": workload_name(w), "value": value, "unit": UNIT, "steps": K, "warmup": W,
+           "ms_per_step": ms / K, "gpu_launches": int(launches), "clocks": clocks.summary(),
+           "residual_last": float(hist[-1]) if len(hist) else None, "medium_generation_s": t_gen,
+           "whole_step": {"floor_ledger_bytes_per_voxel_iteration": floor_bytes / w.voxels,
+                          "achieved": floor_bytes * per_s / world, "frac": floor_bytes * per_s / world / peak,
+                          "sparse_source_ledger_bytes_per_voxel_iteration": sparse_bytes / w.voxels,
+                          "achieved_sparse_source": sparse_bytes * per_s / world,
+                          "frac_sparse_source": sparse_bytes * per_s / world / peak,
+                          "note": "frac = floor ledger (SURVEY 8(d), the quoted denominator); frac_sparse_source = the bytes "
+                                  "this workload must move (all-zero rows of y are skipped); peak = " + peak_kind},
+           "kernels": kernels, "kernels_above_peak": [k["name"] for k in kernels if k["GBps"] > peak],
+           "kernel_times": "CUDA events around every launch, " + ("inside the timed region" if profile_in_timed_region
+                           else "second pass of the same K steps (the timed region replays CUDA graphs)"),
+           "_stats": stats, "_peak": (peak, peak_kind)}
+    return s, w, yd, xd, res
+
+
+def primary_line(res, w, world, unfused):
+    """The contract's JSON line from the result of the primary workload."""
+    stats, (peak, peak_kind) = res.pop("_stats"), res.pop("_peak")
     top = stats[0]
     top_ms = top["total_ms"] / top["launches"]
     top_bytes = top["algorithmic_bytes"] / top["launches"]
     achieved = top_bytes / (top_ms * 1e-3) / 1e9
-    info = s.info()
-    alg_bytes_it = info["algorithmic_bytes_per_iteration"]
+    total_kernel_ms = sum(k["total_ms"] for k in stats)
     roofline = {"bound": "hbm", "kernel": top["name"], "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": dominant_kernel_traffic(top["name"], w.voxels), "peak_kind": peak_kind,
+                "frac": achieved / peak, "traffic": dominant_kernel_traffic(top["name"], w.voxels),
+                "traffic_source": TRAFFIC_SOURCE, "peak_kind": peak_kind,
                 "algorithmic_bytes_per_launch": top_bytes, "avg_launch_ms": top_ms,
-                "share_of_step": top["total_ms"] / total_kernel_ms,
-                "kernel_times": "CUDA events around every launch, " + ("inside the timed region" if profile_in_timed_region
-                                else "second pass of the same K steps (the timed region replays CUDA graphs)"),
-                "whole_step": {"algorithmic_bytes_per_voxel_iteration": alg_bytes_it / w.voxels,
-                               "achieved": alg_bytes_it * K / (ms * 1e-3) / 1e9,
-                               "frac": alg_bytes_it * K / (ms * 1e-3) / 1e9 / peak},
-                "kernels": [{"name": k["name"], "launches_per_step": k["launches"] / K,
-                             "avg_ms": k["total_ms"] / k["launches"],
-                             "GBps": k["algorithmic_bytes"] / max(k["total_ms"], 1e-9) / 1e6} for k in stats]}
-
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "c64", "data": "synthetic",
-            "config": {"workload": workload_name(w), "l2": "inputs larger than L2 (%.1f GiB per array)" % (w.voxels * 8 / 2 ** 30)
-                       if w.voxels * 8 > 4 * 126e6 else "arrays comparable to L2; no flush (the step streams 4 arrays)",
-                       "parallelism": "replicas x%d (path does not shard in this build)" % world,
-                       "fused": not args.unfused, "residual_last": float(hist[-1]) if len(hist) else None,
-                       "medium_generation_s": t_gen},
-            "clocks": clocks.summary(), "gpu_launches": int(launches), "roofline": roofline}
-    return s, w, yd, xd, line, rank, world
+                "share_of_step": top["total_ms"] / total_kernel_ms, "kernel_times": res["kernel_times"],
+                "whole_step": res["whole_step"], "kernels": res["kernels"], "kernels_above_peak": res["kernels_above_peak"]}
+    return {"metric": METRIC, "value": res["value"], "unit": UNIT, "n_gpus": world, "steps": res["steps"],
+            "warmup": res["warmup"], "ms_per_step": res["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "c64", "data": "synthetic", "config": config_block(w, world),
+            "run": {"fused": not unfused, "residual_last": res["residual_last"], "medium_generation_s": res["medium_generation_s"]},
+            "clocks": res["clocks"], "gpu_launches": res["gpu_launches"], "roofline": roofline}
 
 
 def add_e2e(s, w, y, line, K):
@@ -316,15 +354,16 @@ def add_e2e(s, w, y, line, K):
     del yh, xh
 
 
-def add_converge(line, dev):
-    """Seconds to converge (BASELINE.json metric, second part): cold-start mbs_solve of config 3 at its tol, and the
+def converge(cfg, dev, with_floor=True):
+    """Seconds to converge (BASELINE.json metric, second part): cold-start mbs_solve of config `cfg` at its tol, and the
     complex64 residual floor of that case (minimum eps when iterating on without a stop test)."""
     import torch
     from paper_2410_02395_b200 import binding, workloads
-    w = workloads.config(3)
+    w = workloads.config(cfg)
     n_map, y = w.make_medium(), w.make_source()
     s = binding.Solver.from_workload(w, device=dev)
-    s.set_potential(n_map)
+    s.set_potential(torch.from_numpy(n_map).to(dev))
+    del n_map
     yd = torch.from_numpy(y).to(dev)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -332,19 +371,24 @@ def add_converge(line, dev):
     torch.cuda.synchronize()
     dt = time.perf_counter() - t0
     loop_ms = s.info()["last_solve_ms"]
-    # complex64 floor: keep iterating without a stop test until eps stops falling (chunks of 500, at most 20 000 more)
-    nu, floor, extra = s.info()["norm_rhs"], float(hist.min()), 0
-    while extra < 20000:
-        chunk_min = float(s.iterate(yd, x, 500, nu=nu).min())
-        extra += 500
-        stalled = chunk_min > 0.98 * floor
-        floor = min(floor, chunk_min)
-        if stalled:
-            break
-    line["time_to_converge"] = {"workload": workload_name(w), "tol": w.tol, "seconds": dt, "iterations": int(len(hist)),
-                                "status": binding.STATUS_NAMES[rc], "device_loop_ms": loop_ms,
-                                "complex64_floor": floor, "floor_iterations_after_stop": extra}
+    out = {"workload": workload_name(w), "tol": w.tol, "seconds": dt, "iterations": int(len(hist)),
+           "status": binding.STATUS_NAMES[rc], "device_loop_ms": loop_ms,
+           "Gvoxel_it_per_s_over_the_solve": w.voxels * len(hist) / (loop_ms * 1e-3) / 1e9,
+           "monotone": bool(np.all(np.diff(hist) <= 0.0)), "residual_final": float(hist[-1])}
+    if with_floor:
+        # complex64 floor: keep iterating without a stop test until eps stops falling (chunks of 500, at most 20 000 more)
+        nu, floor, extra = s.info()["norm_rhs"], float(hist.min()), 0
+        while extra < 20000:
+            chunk_min = float(s.iterate(yd, x, 500, nu=nu).min())
+            extra += 500
+            stalled = chunk_min > 0.98 * floor
+            floor = min(floor, chunk_min)
+            if stalled:
+                break
+        out["complex64_floor"] = floor
+        out["floor_iterations_after_stop"] = extra
     s.close()
+    return out
 
 
 def main():
@@ -352,26 +396,54 @@ def main():
     if args.impl == "reference":
         run_reference(args)
         return
-    s, w, yd, xd, line, rank, world = run_b200(args)
-    K = line["steps"]
-    if rank == 0:
-        if not args.no_e2e:
-            y = yd.cpu().numpy()
-            del xd
-            add_e2e(s, w, y, line, K)
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if args.converge_config is not None:
+        if rank == 0:
+            print(json.dumps({"time_to_converge": converge(args.converge_config, dev, with_floor=args.converge_config == 3)}))
+        return
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = args.config or 5
+    K = args.steps if args.steps is not None else DEFAULT_STEPS[cfg]
+    W = max(args.warmup if args.warmup is not None else 3, 3)
+    shape = tuple(int(v) for v in args.shape.split(",")) if args.shape else None
+    s, w, yd, xd, res = time_config(cfg, K, W, dev, world, shape=shape, unfused=args.unfused)
+    line = primary_line(res, w, world, args.unfused)
+    if rank == 0 and not args.no_e2e:
+        y = yd.cpu().numpy()
+        del xd
+        xd = None
+        add_e2e(s, w, y, line, K)
     s.close()
-    del s, yd
+    del s, yd, xd
+    torch.cuda.empty_cache()
+    # the two other 3-D configs of BASELINE.json ("... >= 70 % of B200 HBM bandwidth on the 3D configs"), same timing
+    if args.config is None and shape is None and not args.no_other_configs:
+        others = []
+        for oc in (3, 4):
+            so, wo, yo, xo, ro = time_config(oc, args.steps if args.steps is not None else DEFAULT_STEPS[oc], W, dev, world)
+            so.close()
+            del so, yo, xo
+            torch.cuda.empty_cache()
+            ro.pop("_stats"), ro.pop("_peak")
+            others.append(ro)
+        line["other_configs"] = others
     if rank == 0:
-        import torch
-        torch.cuda.empty_cache()
         if not args.no_converge:
-            add_converge(line, torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0"))))
+            line["time_to_converge"] = converge(3, dev)
         if not args.no_cpu_baseline and world == 1:
-            r = oracle_sample(args.config, 6)
+            r = oracle_sample(cfg, 3, full=args.cpu_baseline_full, budget_s=3600.0 if args.cpu_baseline_full else 25.0)
             line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
         print(json.dumps(line))
     if world > 1:
-        import torch.distributed as dist
         dist.barrier()
         dist.destroy_process_group()
 

@@ -102,6 +102,9 @@ typedef struct mbs_info {
     uint64_t workspace_bytes;
     int64_t kernel_launches;       /* kernels launched by this context so far                        */
     double last_solve_ms;          /* device time of the last mbs_solve* iteration loop (CUDA events) */
+    double sparse_source_bytes_per_iteration; /* the ledger minus the all-zero rows of the last source, which the first
+                                      sweep does not read (SURVEY 8(d) "source stored sparsely": 104 B/voxel for a
+                                      point source); equals the floor ledger before the first solve            */
 } mbs_info;
 
 /*

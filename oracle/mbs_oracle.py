@@ -20,6 +20,7 @@ Readings of points the paper leaves open (listed in DESIGN.md section 3, after S
   R7  residual normalised by the global ||Gamma^-1 y||.
   R8  eps_n belongs to x^(n); the update is applied before the stop test.
   R9  p = 2 pi fftfreq(M, h); forward unnormalised, inverse 1/M.
+  R17 subdomain activation (the paper gives neither the norm nor the threshold): see solve_activated.
 
 Pins (tests/test_oracle_pins.py, `-m "not gpu"`): printed K_t / sigma_max values, Eq. (9) -> Eq. (4),
 dense assembly from explicit DFT matrices, dense direct solve, monotone residual, eps_0 = 1,
@@ -231,6 +232,61 @@ class MBSOracle:
             if eps < tol:
                 break
         return x, np.asarray(history)
+
+
+# ---- subdomain activation, reading R17 --------------------------------------------------
+def _subdomain_slices(o):
+    return [tuple(slice(i * m, (i + 1) * m) for i, m in zip(idx, o.M)) for idx in np.ndindex(*o.S)]
+
+
+def solve_activated(o, y, x0=None, tol=1e-6, max_iter=1000, threshold=None, callback=None):
+    """Eq. (6) with the activation strategy of P:139-141: "initially activating only those subdomains that hold
+    a source term.  Neighbouring subdomains are activated only after the norm of the transferred field exceeds a
+    certain threshold."  The paper fixes neither the norm nor the threshold; reading R17:
+
+      * a subdomain is active from the start if y or x^(0) is non-zero anywhere in it;
+      * before update n, an inactive subdomain s becomes active (and stays so) if
+            T_s := sqrt( sum_d || (corr_d x^(n)) restricted to s ||_2^2 )  >=  threshold * nu,
+        corr_d = the edge corrections of step 10 (an inactive subdomain holds x_s = 0, so what lands in it is exactly
+        the field its neighbours transfer, P:126 step 2), nu = ||Gamma^-1 y_vec|| the normalisation of the residual
+        (P:130).  Default threshold = tol / 10: what an inactive subdomain would add to the relative residual stays an
+        order of magnitude below the stopping threshold;
+      * an inactive subdomain is not computed: it contributes d_s = 0, receives no update and no residual.
+    threshold = 0 activates every subdomain at n = 0 and reproduces `solve` exactly.
+    Returns (x, residual_history, activation_iteration per subdomain in np.ndindex(S) order; -1 = never)."""
+    if threshold is None:
+        threshold = 0.1 * tol
+    y_vec = -o.c * np.asarray(y).astype(np.complex128)
+    x = np.zeros(o.shape, dtype=np.complex128) if x0 is None else np.asarray(x0).astype(np.complex128).copy()
+    nu = np.linalg.norm(o.apply_B(o.propagate(y_vec)))
+    blocks = _subdomain_slices(o)
+    active = [bool(np.any(y_vec[sl] != 0) or np.any(x[sl] != 0)) for sl in blocks]
+    activated_at = [0 if a else -1 for a in active]
+    history = []
+    for n in range(max_iter):
+        if not all(active):
+            corr = [o.corr_axis(x, d) for d in range(o.ndim)]
+            for k, sl in enumerate(blocks):
+                if not active[k]:
+                    T = np.sqrt(sum(np.linalg.norm(cd[sl]) ** 2 for cd in corr))
+                    if T >= threshold * nu:
+                        active[k] = True
+                        activated_at[k] = n
+        mask = np.zeros(o.shape, dtype=np.float64)
+        for k, sl in enumerate(blocks):
+            if active[k]:
+                mask[sl] = 1.0
+        u = o.propagate(o.apply_B(x) + y_vec)
+        d = (x - u) * mask
+        r = o.apply_B(d) * mask
+        eps = float(np.linalg.norm(r) / nu)
+        history.append(eps)
+        x = x - ALPHA * r
+        if callback is not None:
+            callback(n, eps, x)
+        if eps < tol:
+            break
+    return x, np.asarray(history), activated_at
 
 
 def from_workload(w, n_map=None):

@@ -48,7 +48,7 @@ class mbs_info(ctypes.Structure):
                 ("alpha", ctypes.c_double), ("norm_rhs", ctypes.c_double),
                 ("algorithmic_bytes_per_iteration", ctypes.c_double),
                 ("workspace_bytes", ctypes.c_uint64), ("kernel_launches", ctypes.c_int64),
-                ("last_solve_ms", ctypes.c_double)]
+                ("last_solve_ms", ctypes.c_double), ("sparse_source_bytes_per_iteration", ctypes.c_double)]
 
 
 class mbs_kernel_stat(ctypes.Structure):

@@ -75,6 +75,7 @@ struct mbs_ctx {
     cd c = 0, k02 = 0;
     double v_max = 0, norm_A12 = 0, beta = 0.5, alpha = 0.75, norm_rhs = 0, last_solve_ms = 0;
     int sum_a = 0;
+    double y_row_fraction = 1.0;     // fraction of the grid rows of the last source that are not all zero (sweep 1 skips the rest)
     bool potential_set = false;
     std::vector<double> Kh;  // t*t
 
@@ -673,7 +674,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     if (c->ndim == 1) {
         p.slot0 = 0; p.finish = 1;
         p.n_total = e->fused_blocks(FUSED_1D, g.t, p.n_tiles, c->num_sms);
-        KernelScope ks(c, "fused_1d", 4 * vb);
+        KernelScope ks(c, "fused_1d", (3.0 + c->y_row_fraction) * vb);
         MBS_CUDA(c, e->fused(p, c->tw_dev[2], FUSED_1D, done, c->num_sms, c->stream));
         return MBS_OK;
     }
@@ -687,7 +688,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
                              ? e->merged_blocks(g.S[2], g.t, p.n_lines, c->num_sms) : 0;
         const bool merge = nb51 > 0;
         if (!(merge && c->u_ready)) {
-            KernelScope ks(c, "line_sweep1", 4 * vb);
+            KernelScope ks(c, "line_sweep1", (3.0 + c->y_row_fraction) * vb);     // all-zero rows of y are not read
             MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S1, done, c->num_sms, c->stream));
         } else if (mask01) {
             // u of the rows outside the slabs was written by the merged sweep of the iteration before; the slab rows
@@ -759,7 +760,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
         return MBS_OK;
     }
     {
-        KernelScope ks(c, "fused_sweep1", 4 * vb);                                    // reads x, B_diag, y; writes u
+        KernelScope ks(c, "fused_sweep1", (3.0 + c->y_row_fraction) * vb);           // reads x, B_diag, y (non-empty rows); writes u
         MBS_CUDA(c, e->fused(p, c->tw_dev[2], FUSED_S1, done, c->num_sms, c->stream));
     }
     MBS_TRY(run_middle_sweeps(c, c->u, 1, true));
@@ -840,6 +841,15 @@ static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, do
         MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
     }
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));   // state_pinned[0] is reused by the poll loop
+    {
+        // rows of y the first sweep has to read (byte ledger of the sparse-source row of SURVEY 8(d))
+        const size_t rows = (size_t)(c->g.voxels / c->g.N[2]);
+        std::vector<unsigned char> m(rows);
+        MBS_CUDA(c, cudaMemcpy(m.data(), c->ymask, rows, cudaMemcpyDeviceToHost));
+        size_t nz = 0;
+        for (size_t i = 0; i < rows; ++i) nz += m[i] ? 1 : 0;
+        c->y_row_fraction = rows ? (double)nz / (double)rows : 1.0;
+    }
     if (!(nu > 0)) {
         // the relative residual of P:130 divides by ||Gamma^-1 y_vec||: a zero (or non-finite) source has none
         DevState st{};
@@ -1072,6 +1082,8 @@ extern "C" int mbs_get_info(const mbs_ctx* c, mbs_info* out) {
     out->alpha = c->alpha; out->norm_rhs = c->norm_rhs;
     const double per_voxel = c->ndim == 3 ? 112.0 : (c->ndim == 2 ? 80.0 : 32.0);
     out->algorithmic_bytes_per_iteration = per_voxel * (double)c->g.voxels;
+    // the same ledger when the all-zero rows of the source are not read ("source stored sparsely": 104 B)
+    out->sparse_source_bytes_per_iteration = (per_voxel - 8.0 * (1.0 - c->y_row_fraction)) * (double)c->g.voxels;
     out->workspace_bytes = c->ws_bytes;
     out->kernel_launches = c->launches;
     out->last_solve_ms = c->last_solve_ms;

@@ -17,9 +17,9 @@ def test_reference_arm_prints_one_valid_json_line():
     assert d["impl"] == "reference" and d["metric"].startswith("Gvoxel-iterations/s") and d["unit"] == "Gvoxel-it/s"
     assert d["higher_is_better"] is True and d["vs_baseline"] is None and d["data"] == "synthetic"
     assert d["steps"] == 2 and d["warmup"] == 1 and d["value"] > 0 and d["ms_per_step"] > 0
-    assert d["config"]["workload"].startswith("cfg3_256x256x256") and "sample" in d["config"]
+    assert d["config"]["workload"].startswith("cfg3_256x256x256") and "l2" in d["config"] and "parallelism" in d["config"]
     cb = d["cpu_baseline"]
-    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] == d["value"] and "oracle iterations" in cb["sample"]
+    assert cb["kind"] == "oracle" and cb["cores"] >= 1 and cb["value"] == d["value"] and "oracle iteration" in cb["sample"]
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
 
 

@@ -356,3 +356,80 @@ def test_config1_iterations_and_split_ratio():
     # the two decompositions solve the same problem up to the truncation (1.7e-4 squared metric)
     err_sq = np.linalg.norm(x2 - x1) ** 2 / np.linalg.norm(x1) ** 2
     assert err_sq < 5e-3
+
+
+# ------------------------------------------------------------------------------------------
+# subdomain activation (reading R17 in DESIGN.md section 3)
+# ------------------------------------------------------------------------------------------
+def _activation_case():
+    N = 512
+    n = np.ones(N, dtype=np.complex64)
+    n[200:260] = 1.3 + 0.01j
+    o = orc.MBSOracle(n, 0.25, 1.0, (16,), (4,), n_correction=8)
+    y = np.zeros(N, dtype=np.complex128)
+    y[40] = 1.0
+    return o, y
+
+
+def test_activation_threshold_zero_is_the_plain_iteration():
+    """R17: with threshold 0 every subdomain is active from n = 0, and the activated iteration IS Eq. (6)."""
+    o, y = _activation_case()
+    x0, h0 = o.solve(y, tol=1e-4, max_iter=20000)
+    x1, h1, act = orc.solve_activated(o, y, tol=1e-4, max_iter=20000, threshold=0.0)
+    assert act == [0, 0, 0, 0]
+    assert np.array_equal(x1, x0) and np.array_equal(h1, h0)
+
+
+def test_activation_converges_to_the_same_field():
+    """"Although this initially causes a small error, the MBS converges to the correct solution from any
+    starting point and thus nullifies these errors."  Only the source-holding subdomain starts active; the others
+    follow in order of their distance from the source; the converged field agrees with the plain iteration far below
+    the stopping threshold and the iteration count is unchanged within 1 %; work is saved (12 % in the paper)."""
+    o, y = _activation_case()
+    tol = 1e-4
+    x0, h0 = o.solve(y, tol=tol, max_iter=20000)
+    held = {}
+
+    def cb(n, eps, x):
+        # subdomains 2 and 3 hold exactly zero until they are activated
+        held[n] = (bool(np.all(x[256:384] == 0)), bool(np.all(x[384:512] == 0)))
+
+    x1, h1, act = orc.solve_activated(o, y, tol=tol, max_iter=20000, callback=cb)
+    assert act[0] == 0 and all(a > 0 for a in act[1:])
+    assert act[1] <= act[2] <= act[3]                      # the field reaches them in order of distance
+    assert all(held[n][0] for n in range(act[2] - 1)) and not held[act[2]][0]
+    assert all(held[n][1] for n in range(act[3] - 1)) and not held[act[3]][1]
+    assert np.linalg.norm(x1 - x0) / np.linalg.norm(x0) < 0.1 * tol
+    assert abs(len(h1) - len(h0)) <= 0.01 * len(h0)
+    saved = 1.0 - sum(len(h1) - a for a in act) / (len(act) * len(h1))
+    assert saved > 0.01
+    # a larger threshold delays activation and saves more work; the field still agrees at the level of the threshold
+    x2, h2, act2 = orc.solve_activated(o, y, tol=tol, max_iter=20000, threshold=10 * tol)
+    assert all(b >= a for a, b in zip(act, act2)) and act2[3] > act[3]
+    assert np.linalg.norm(x2 - x0) / np.linalg.norm(x0) < 30 * tol
+
+
+def test_activation_rule_against_dense_transfer_norm():
+    """R17 rule, checked against the dense correction matrices of tests/dense_reference.py: an inactive subdomain s is
+    activated before the first update n at which sqrt(sum_d ||(c C_d x^(n))_s||^2) >= threshold * nu, where C_d holds the
+    K_t entries placed by index and nu = ||B (L+I)^-1 y_vec||."""
+    shape, S, t = (16, 12), (2, 2), 3
+    o = _small_oracle(shape, S, (2, 2), t, seed=51)
+    L, V = dr.assemble(o.k2, o.k02, o.c, shape, S, t, o.h, o.a, (0, 0))
+    I = np.eye(L.shape[0])
+    Cd = [o.c * dr.kron_axis(dr.axis_correction_matrix(shape[d], S[d], t, o.h, False), shape, d) for d in range(2)]
+    y = np.zeros(shape, dtype=np.complex128)
+    y[2, 2] = 1.0                                           # subdomain (0, 0)
+    nu = np.linalg.norm((I - V) @ np.linalg.solve(L + I, (-o.c * y).reshape(-1)))
+    thr = 3e-2
+    xs = {}
+    x, hist, act = orc.solve_activated(o, y, tol=1e-6, max_iter=400, threshold=thr,
+                                       callback=lambda n, eps, xx: xs.__setitem__(n + 1, xx.copy()))
+    xs[0] = np.zeros(shape, dtype=np.complex128)
+    blocks = [(slice(0, 8), slice(0, 6)), (slice(0, 8), slice(6, 12)), (slice(8, 16), slice(0, 6)), (slice(8, 16), slice(6, 12))]
+    assert act[0] == 0 and all(a > 0 for a in act[1:])
+    for k in range(1, 4):
+        def T(n):
+            return np.sqrt(sum(np.linalg.norm((C @ xs[n].reshape(-1)).reshape(shape)[blocks[k]]) ** 2 for C in Cd))
+        assert T(act[k]) >= thr * nu                        # activated when the transferred norm reaches the threshold
+        assert all(T(n) < thr * nu for n in range(act[k]))  # ... and not before
