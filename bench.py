@@ -46,8 +46,9 @@ UNIT = "Gvoxel-it/s"
 # 10-30 s budget of this leg; `--cpu-baseline-full` times the oracle on the workload itself when the host has the memory.
 SAMPLE_GRIDS = {3: ((256, 256, 256), (2, 1, 1), (16, 16, 16)),
                 4: ((320, 320, 320), (1, 1, 1), (24, 24, 24)),
-                5: ((256, 512, 512), (1, 1, 1), (32, 32, 32))}
-DEFAULT_STEPS = {3: 400, 4: 60, 5: 30}
+                5: ((256, 512, 512), (1, 1, 1), (32, 32, 32)),
+                6: ((630, 315, 315), (2, 1, 1), (20, 20, 20))}
+DEFAULT_STEPS = {3: 400, 4: 60, 5: 30, 6: 20}
 
 
 def parse_args():
@@ -55,9 +56,10 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=None)
     ap.add_argument("--warmup", type=int, default=None)
-    ap.add_argument("--config", type=int, default=None, choices=(3, 4, 5),
-                    help="workload (default 5; without this flag configs 3 and 4 are timed too, under other_configs)")
-    ap.add_argument("--converge-config", type=int, default=None, choices=(3, 4, 5),
+    ap.add_argument("--config", type=int, default=None, choices=(3, 4, 5, 6),
+                    help="workload (default 5; without this flag configs 3 and 4 are timed too, under other_configs); "
+                         "6 = the shape of the paper's own large run, 1260^3 voxels in two subdomains (context, not a BASELINE config)")
+    ap.add_argument("--converge-config", type=int, default=None, choices=(3, 4, 5, 6),
                     help="only: cold-start mbs_solve of this config at its tol; prints seconds and iterations")
     ap.add_argument("--cpu-baseline-full", action="store_true",
                     help="time the oracle on the workload itself (3 iterations; config 5 needs ~120 GiB of host memory)")
@@ -68,6 +70,11 @@ def parse_args():
     ap.add_argument("--no-converge", action="store_true")
     ap.add_argument("--no-other-configs", action="store_true", help="default run: do not time configs 3 and 4 as well")
     ap.add_argument("--unfused", action="store_true", help="one kernel per step of P:122-128 instead of the fused sweeps")
+    ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
+                    help="kernel option for profiling runs, e.g. MERGE=1, LINE=0, TMA=0 (enum mbs_option; not the headline)")
+    ap.add_argument("--activation", type=float, default=None, metavar="THRESHOLD",
+                    help="--converge-config only: solve with subdomain activation (P:139-141) at this relative threshold "
+                         "(negative: the default tol / 10) and report it beside the plain solve")
     return ap.parse_args()
 
 
@@ -354,7 +361,7 @@ def add_e2e(s, w, y, line, K):
     del yh, xh
 
 
-def converge(cfg, dev, with_floor=True):
+def converge(cfg, dev, with_floor=True, activation=None):
     """Seconds to converge (BASELINE.json metric, second part): cold-start mbs_solve of config `cfg` at its tol, and the
     complex64 residual floor of that case (minimum eps when iterating on without a stop test)."""
     import torch
@@ -364,6 +371,8 @@ def converge(cfg, dev, with_floor=True):
     s = binding.Solver.from_workload(w, device=dev)
     s.set_potential(torch.from_numpy(n_map).to(dev))
     del n_map
+    if activation is not None:
+        s.set_activation(True, activation)
     yd = torch.from_numpy(y).to(dev)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -375,6 +384,11 @@ def converge(cfg, dev, with_floor=True):
            "status": binding.STATUS_NAMES[rc], "device_loop_ms": loop_ms,
            "Gvoxel_it_per_s_over_the_solve": w.voxels * len(hist) / (loop_ms * 1e-3) / 1e9,
            "monotone": bool(np.all(np.diff(hist) <= 0.0)), "residual_final": float(hist[-1])}
+    if activation is not None:
+        act = s.activation()
+        out["activation"] = {"threshold": activation if activation >= 0 else 0.1 * w.tol, "activated_at": act,
+                             "work_fraction": sum(len(hist) - a for a in act if a >= 0) / (len(act) * len(hist)),
+                             "reading": "R17 (DESIGN.md section 3); P:139-141 reports 12 % on 100^3 wavelengths, 3x1x1"}
     if with_floor:
         # complex64 floor: keep iterating without a stop test until eps stops falling (chunks of 500, at most 20 000 more)
         nu, floor, extra = s.info()["norm_rhs"], float(hist.min()), 0
@@ -407,7 +421,11 @@ def main():
     dev = torch.device("cuda", local)
     if args.converge_config is not None:
         if rank == 0:
-            print(json.dumps({"time_to_converge": converge(args.converge_config, dev, with_floor=args.converge_config == 3)}))
+            out = {"time_to_converge": converge(args.converge_config, dev, with_floor=args.converge_config == 3)}
+            if args.activation is not None:
+                out["time_to_converge_with_activation"] = converge(args.converge_config, dev, with_floor=False,
+                                                                   activation=args.activation)
+            print(json.dumps(out))
         return
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
@@ -415,7 +433,9 @@ def main():
     K = args.steps if args.steps is not None else DEFAULT_STEPS[cfg]
     W = max(args.warmup if args.warmup is not None else 3, 3)
     shape = tuple(int(v) for v in args.shape.split(",")) if args.shape else None
-    s, w, yd, xd, res = time_config(cfg, K, W, dev, world, shape=shape, unfused=args.unfused)
+    from paper_2410_02395_b200 import binding as _b
+    options = [(getattr(_b, "MBS_OPT_" + kv.split("=")[0].upper()), int(kv.split("=")[1])) for kv in args.opt]
+    s, w, yd, xd, res = time_config(cfg, K, W, dev, world, shape=shape, unfused=args.unfused, options=options)
     line = primary_line(res, w, world, args.unfused)
     if rank == 0 and not args.no_e2e:
         y = yd.cpu().numpy()

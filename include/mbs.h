@@ -75,6 +75,10 @@ enum mbs_option {
     MBS_OPT_MERGE = 6,          /* 1: the last sweep also runs the next iteration's first sweep on every row outside the
                                    axis-0/1 slabs (saves the re-read of x and B_diag, 96 B ledger); needs MBS_OPT_LINE.
                                    Default 0: with 128 registers per thread it is latency-bound and measured slower  */
+    MBS_OPT_REFINE = 7,         /* split iterate x = x_ref + delta (api.cu recenter()): the FFT sweeps run on the small part
+                                   delta, so the complex64 rounding floor of the residual falls with it and tolerances such
+                                   as config 1's 1e-6 are reachable; same iteration in exact arithmetic, two extra arrays.
+                                   -1 (default): on for grids of <= 2^21 voxels; 0: off; 1: on                   */
     MBS_OPT_PROFILE = 3         /* 1: bracket every kernel launch with CUDA events on the context's stream and
                                    accumulate per-kernel device time (mbs_get_kernel_stats); disables graphs   */
 };
@@ -183,6 +187,27 @@ MBS_API int mbs_iterate(mbs_ctx* ctx, const void* y_device, void* x_device, int3
  * copies x back.  The end-to-end entry point (bench.py "e2e"). */
 MBS_API int mbs_solve_host(mbs_ctx* ctx, const void* y_host, void* x_host, double tol, int32_t max_iter,
                    double* residual_history, int32_t* n_iter);
+
+/*
+ * Subdomain activation ("initially activating only those subdomains that hold a source term.  Neighbouring
+ * subdomains are activated only after the norm of the transferred field exceeds a certain threshold").  The paper
+ * fixes neither the norm nor the threshold; reading R17, the same rule as the oracle's
+ * solve_activated:
+ *   - a subdomain is active from the start if y or x^(0) is non-zero anywhere in it;
+ *   - before update n an inactive subdomain s becomes active (for good) when
+ *       sqrt( sum_d || (corr_d x^(n)) restricted to s ||^2 ) >= threshold * ||Gamma^-1 y_vec||,
+ *     corr_d = the edge corrections of P:124-128 (x_s = 0 there, so this is what its neighbours transfer into it);
+ *   - an inactive subdomain is not computed: no FFT, no update, no residual.
+ *  enable     0 / 1 (default 0).
+ *  threshold  relative to ||Gamma^-1 y_vec||; < 0: tol / 10 of the solve (0 for mbs_iterate, i.e. all active).
+ * Needs a 2-D or 3-D grid and the default kernel options.  Errors: MBS_ERR_INVALID_ARG, MBS_ERR_UNSUPPORTED_SIZE, MBS_ERR_OOM.
+ */
+MBS_API int mbs_set_activation(mbs_ctx* ctx, int enable, double threshold);
+
+/* Iteration at which each subdomain was activated in the last solve (index (s0*S1 + s1)*S2 + s2 in the order of
+ * n_subdomains; 0 = from the start, -1 = never; all 0 when activation is off).  activated_at: host, `capacity` entries,
+ * may be NULL; *n_subdomains receives the number of subdomains. */
+MBS_API int mbs_get_activation(const mbs_ctx* ctx, int32_t* activated_at, int32_t capacity, int32_t* n_subdomains);
 
 MBS_API int mbs_get_info(const mbs_ctx* ctx, mbs_info* out);
 

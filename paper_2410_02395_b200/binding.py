@@ -29,6 +29,7 @@ MBS_ERR_CUDA, MBS_ERR_NOT_CONVERGED, MBS_ERR_NUMERIC, MBS_ERR_STATE = 4, 5, 6, 7
 MBS_OP_B, MBS_OP_PROPAGATOR, MBS_OP_A, MBS_OP_PRECOND_A = 0, 1, 2, 3
 MBS_OPT_FUSED, MBS_OPT_CHECK_INTERVAL, MBS_OPT_USE_GRAPH, MBS_OPT_PROFILE, MBS_OPT_TMA, MBS_OPT_LINE = 0, 1, 2, 3, 4, 5
 MBS_OPT_MERGE = 6
+MBS_OPT_REFINE = 7
 
 STATUS_NAMES = {0: "MBS_OK", 1: "MBS_ERR_INVALID_ARG", 2: "MBS_ERR_UNSUPPORTED_SIZE", 3: "MBS_ERR_OOM",
                 4: "MBS_ERR_CUDA", 5: "MBS_ERR_NOT_CONVERGED", 6: "MBS_ERR_NUMERIC", 7: "MBS_ERR_STATE"}
@@ -36,7 +37,8 @@ STATUS_NAMES = {0: "MBS_OK", 1: "MBS_ERR_INVALID_ARG", 2: "MBS_ERR_UNSUPPORTED_S
 # every symbol include/mbs.h declares (tests/test_abi.py checks the library exports them all)
 DECLARED_SYMBOLS = ("mbs_create", "mbs_fft_supported", "mbs_workspace_bytes", "mbs_set_workspace", "mbs_set_option",
                     "mbs_set_potential", "mbs_apply_operator", "mbs_solve", "mbs_solve_host", "mbs_iterate",
-                    "mbs_get_info", "mbs_get_kernel_stats", "mbs_reset_kernel_stats", "mbs_destroy", "mbs_last_error")
+                    "mbs_get_info", "mbs_get_kernel_stats", "mbs_reset_kernel_stats", "mbs_destroy", "mbs_last_error",
+                    "mbs_set_activation", "mbs_get_activation")
 
 
 class mbs_info(ctypes.Structure):
@@ -84,6 +86,10 @@ _lib.mbs_get_kernel_stats.argtypes = [_vp, ctypes.POINTER(mbs_kernel_stat), ctyp
 _lib.mbs_get_kernel_stats.restype = ctypes.c_int
 _lib.mbs_reset_kernel_stats.argtypes = [_vp]
 _lib.mbs_reset_kernel_stats.restype = ctypes.c_int
+_lib.mbs_set_activation.argtypes = [_vp, ctypes.c_int, ctypes.c_double]
+_lib.mbs_set_activation.restype = ctypes.c_int
+_lib.mbs_get_activation.argtypes = [_vp, ctypes.POINTER(ctypes.c_int32), ctypes.c_int32, ctypes.POINTER(ctypes.c_int32)]
+_lib.mbs_get_activation.restype = ctypes.c_int
 _lib.mbs_get_info.argtypes = [_vp, ctypes.POINTER(mbs_info)]
 _lib.mbs_get_info.restype = ctypes.c_int
 _lib.mbs_destroy.argtypes = [_vp]
@@ -193,6 +199,19 @@ def mbs_reset_kernel_stats(ctx):
     _check(ctx, _lib.mbs_reset_kernel_stats(ctx))
 
 
+def mbs_set_activation(ctx, enable: bool, threshold: float = -1.0):
+    _check(ctx, _lib.mbs_set_activation(ctx, int(bool(enable)), float(threshold)))
+
+
+def mbs_get_activation(ctx) -> list:
+    """Iteration at which each subdomain was activated in the last solve (subdomains in np.ndindex(S) order)."""
+    n = ctypes.c_int32(0)
+    _check(ctx, _lib.mbs_get_activation(ctx, None, 0, ctypes.byref(n)))
+    arr = (ctypes.c_int32 * max(n.value, 1))()
+    _check(ctx, _lib.mbs_get_activation(ctx, arr, n.value, ctypes.byref(n)))
+    return [int(arr[i]) for i in range(n.value)]
+
+
 def mbs_get_info(ctx) -> dict:
     info = mbs_info()
     _check(ctx, _lib.mbs_get_info(ctx, ctypes.byref(info)))
@@ -294,6 +313,12 @@ class Solver:
     def iterate(self, y_dev, x_dev, n_iter: int, nu: float = 0.0, want_history: bool = True):
         """y_dev, x_dev: complex64 device tensors of the grid shape; x_dev is updated in place."""
         return mbs_iterate(self.ctx, y_dev.data_ptr(), x_dev.data_ptr(), n_iter, nu, want_history)
+
+    def set_activation(self, enable: bool, threshold: float = -1.0):
+        mbs_set_activation(self.ctx, enable, threshold)
+
+    def activation(self) -> list:
+        return mbs_get_activation(self.ctx)
 
     def kernel_stats(self) -> list:
         return mbs_get_kernel_stats(self.ctx)

@@ -27,7 +27,7 @@ FLAGS = ["-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo"
 
 def fft_sizes():
     text = open(os.path.join(CSRC, "fft_plans.h")).read()
-    body = text.split("#define MBS_FOR_EACH_FFT_SIZE(X)")[1]
+    body = text.split("#define MBS_FOR_EACH_FFT_SIZE(X)")[-1].split("#endif")[0]
     return [int(m) for m in re.findall(r"X\((\d+)\)", body)]
 
 
@@ -64,13 +64,20 @@ def _compile(job):
     return obj
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    """Compiles what changed (one digest per object over the source, the headers it includes and the flags) and links."""
+def build(force: bool = False, verbose: bool = False, sizes=None) -> str:
+    """Compiles what changed (one digest per object over the source, the headers it includes and the flags) and links.
+    `sizes` (kernel development only: `--sizes 256,512`) links a library that knows just those subdomain lengths."""
     os.makedirs(OBJDIR, exist_ok=True)
     jobs = []
-    for name in ("api.cu", "kernels.cu", "fft_registry.cu"):
+    for name in ("api.cu", "kernels.cu"):
         jobs.append((os.path.join(CSRC, name), os.path.join(OBJDIR, name[:-3] + ".o"), []))
-    for m in fft_sizes():
+    if sizes:
+        tag = "_".join(str(m) for m in sizes)
+        jobs.append((os.path.join(CSRC, "fft_registry.cu"), os.path.join(OBJDIR, "fft_registry_dev_%s.o" % tag),
+                     ["-DMBS_DEV_SIZES=" + " ".join("X(%d)" % m for m in sizes)]))
+    else:
+        jobs.append((os.path.join(CSRC, "fft_registry.cu"), os.path.join(OBJDIR, "fft_registry.o"), []))
+    for m in (sizes or fft_sizes()):
         jobs.append((os.path.join(CSRC, "fft_inst.cu"), os.path.join(OBJDIR, "fft_%d.o" % m),
                      ["-DMBS_FFT_SIZE=%d" % m]))
     stale, digests = [], {}
@@ -79,7 +86,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
         stamp = obj + ".digest"
         if force or not os.path.exists(obj) or not os.path.exists(stamp) or open(stamp).read() != digests[obj]:
             stale.append((src, obj, extra))
-    if not stale and os.path.exists(LIB):
+    marker = os.path.join(OBJDIR, "linked.txt")
+    linked = " ".join(obj for _, obj, _ in jobs)
+    if not stale and os.path.exists(LIB) and os.path.exists(marker) and open(marker).read() == linked:
         return LIB
     with concurrent.futures.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         list(ex.map(_compile, stale))
@@ -91,10 +100,15 @@ def build(force: bool = False, verbose: bool = False) -> str:
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("link failed: %s\n%s\n%s" % (" ".join(cmd), r.stdout, r.stderr))
+    with open(marker, "w") as f:
+        f.write(linked)
     if verbose:
         print("built %s (%d of %d objects recompiled)" % (LIB, len(stale), len(jobs)))
     return LIB
 
 
 if __name__ == "__main__":
-    build(force="--force" in sys.argv, verbose=True)
+    _sizes = None
+    if "--sizes" in sys.argv:
+        _sizes = [int(v) for v in sys.argv[sys.argv.index("--sizes") + 1].split(",")]
+    build(force="--force" in sys.argv, verbose=True, sizes=_sizes)

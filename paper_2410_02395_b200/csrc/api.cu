@@ -91,12 +91,28 @@ struct mbs_ctx {
     int profile = 0;
     Profiler prof;
 
+    // split iterate x = x_ref + delta (lifts the complex64 residual floor on small grids; see recenter())
+    int refine = -1;                 // MBS_OPT_REFINE: -1 automatic (grids of <= 2^21 voxels), 0 off, 1 on
+    cf* delta = nullptr;             // owned: the small part of the iterate
+    cf* dref = nullptr;              // owned: d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec)
+    bool split = false;              // the running solve iterates on delta
+    double split_eps = 1.0;          // eps at the last re-centering
+    int n_recenter = 0;
+
+    // subdomain activation (R17)
+    int activation = 0;
+    double act_threshold = -1.0;     // relative to nu; < 0: tol / 10 of the solve
+    ActivationState act{};
+    void* act_mem = nullptr;
+    int n_sub = 1;
+    std::vector<int32_t> act_iter_host;
+
     // CUDA graph of one poll interval of iterations (small grids are launch-bound)
     cudaGraphExec_t graph_exec = nullptr;
     cudaStream_t cap_stream = nullptr;   // capture happens on a private stream (the caller's may be the default stream)
     const void* graph_y = nullptr;
     const void* graph_x = nullptr;
-    int graph_batch = 0, graph_fused = -1, graph_tma = -1, graph_line = -1;
+    int graph_batch = 0, graph_fused = -1, graph_tma = -1, graph_line = -1, graph_split = -1;
     int64_t launches_per_batch = 0;
 
     int64_t launches = 0;
@@ -311,6 +327,7 @@ extern "C" int mbs_create(mbs_ctx** out, int ndim, const int64_t* shape, double 
     if (rc == MBS_OK && g.voxels >= (1LL << 31)) rc = fail(nullptr, MBS_ERR_INVALID_ARG, "grid has %lld voxels; the limit is 2^31 - 1", g.voxels);
     if (rc != MBS_OK) { delete c; return rc; }
     c->sum_a = g.a[0] + g.a[1] + g.a[2];
+    c->n_sub = g.S[0] * g.S[1] * g.S[2];
 
     // K_t / h^2 and ||A_12|| (R4, R5)
     const int t = g.t;
@@ -415,6 +432,9 @@ extern "C" void mbs_destroy(mbs_ctx* c) {
     for (cudaEvent_t e : c->prof.pool) cudaEventDestroy(e);
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+    if (c->act_mem) cudaFree(c->act_mem);
+    if (c->delta) cudaFree(c->delta);
+    if (c->dref) cudaFree(c->dref);
     delete c;
 }
 
@@ -456,8 +476,47 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
         case MBS_OPT_TMA: c->use_tma = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_LINE: c->use_line = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_MERGE: c->use_merge = value ? 1 : 0; return MBS_OK;
+        case MBS_OPT_REFINE: c->refine = value < 0 ? -1 : (value ? 1 : 0); invalidate_graph(c); return MBS_OK;
         default: return fail(c, MBS_ERR_INVALID_ARG, "unknown option %d", option);
     }
+}
+
+// ---------------------------------------------------------------------------------------------
+// subdomain activation
+// ---------------------------------------------------------------------------------------------
+static bool fused_available(const mbs_ctx* c);
+static bool activation_effective(const mbs_ctx* c) {
+    return c->activation && c->ndim >= 2 && c->fused && fused_available(c) && c->use_line && c->fft[2]->line &&
+           !c->use_merge && slab_pass_supported(c->g.t);
+}
+
+extern "C" int mbs_set_activation(mbs_ctx* c, int enable, double threshold) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (enable && c->ndim < 2) return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation needs a 2-D or 3-D grid");
+    if (enable && !(c->fft[2]->line && slab_pass_supported(c->g.t)))
+        return fail(c, MBS_ERR_UNSUPPORTED_SIZE, "subdomain activation needs the warp-line sweeps (contiguous subdomain length <= 512... and t in {2, 4, 8, 16})");
+    if (enable && !c->act_mem) {
+        const size_t ints = (size_t)3 * c->n_sub + 2;
+        const size_t bytes = align_up(sizeof(int) * ints) + sizeof(double) * (size_t)c->n_sub * 6 * ACT_CHUNKS;
+        MBS_CUDA(c, cudaMalloc(&c->act_mem, bytes));
+        MBS_CUDA(c, cudaMemset(c->act_mem, 0, bytes));
+        int* ip = (int*)c->act_mem;
+        c->act.flags = ip; c->act.list = ip + c->n_sub; c->act.act_iter = ip + 2 * c->n_sub;
+        c->act.n_act = ip + 3 * c->n_sub; c->act.ticket = (unsigned int*)(ip + 3 * c->n_sub + 1);
+        c->act.partials = (double*)((char*)c->act_mem + align_up(sizeof(int) * ints));
+    }
+    invalidate_graph(c);
+    c->activation = enable ? 1 : 0;
+    c->act_threshold = threshold;
+    return MBS_OK;
+}
+
+extern "C" int mbs_get_activation(const mbs_ctx* c, int32_t* activated_at, int32_t capacity, int32_t* n_subdomains) {
+    if (!c || !n_subdomains) return MBS_ERR_INVALID_ARG;
+    *n_subdomains = c->n_sub;
+    for (int i = 0; i < c->n_sub && i < capacity && activated_at; ++i)
+        activated_at[i] = i < (int)c->act_iter_host.size() ? c->act_iter_host[i] : 0;
+    return MBS_OK;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -592,6 +651,12 @@ static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, b
     const int cs = (mode == FFT_MID) ? e->CSM : e->CS;
     sg.inner = (int)inner; sg.tiles_inner = (int)((inner + cs - 1) / cs);
     sg.n_tiles = outer * g.S[ax] * sg.tiles_inner;
+    if (in_loop && activation_effective(c) && g.M[2] % cs == 0) {
+        // visit only the tiles of the active subdomains (their list lives in device memory)
+        sg.act_list = c->act.list; sg.n_act = c->act.n_act; sg.axis = ax;
+        sg.tps2 = g.M[2] / cs; sg.tiles_per_sub = (ax == 1 ? g.M[0] : g.M[1]) * sg.tps2;
+        sg.S1 = g.S[1]; sg.S2 = g.S[2]; sg.M0 = g.M[0]; sg.M1 = g.M[1]; sg.row_tiles = g.N[2] / cs;
+    }
     SymbolParams s2 = make_symbol(c, inverse);
     s2.tab_axis = c->p2_dev[ax];
     if (mode == FFT_MID) {
@@ -651,12 +716,16 @@ static int run_iteration_unfused(mbs_ctx* c, const cf* y, cf* x) {
 }
 
 // The fused path needs whole grid rows inside one tile of the contiguous-axis kernel.
-static bool fused_available(const mbs_ctx* c) { return c->fft[2]->CC % c->g.S[2] == 0; }
+static bool fused_available(const mbs_ctx* c) { return c->fft[2]->fused != nullptr && c->fft[2]->CC % c->g.S[2] == 0; }
 
 // one iteration of Eq. (6), fused sweeps (112 B/voxel ledger of DESIGN.md section 5)
 static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     const GridDesc& g = c->g;
     const FftEntry* e = c->fft[2];
+    if (c->split) {   // split iterate: the sweeps run on delta with no source; the last sweep adds d_ref (recenter())
+        y = nullptr;
+        x = c->delta;
+    }
     const int e0 = g.a[0] > 0, e1 = g.a[1] > 0;
     const int* done = &c->state->done;
     FusedParams p{};
@@ -670,6 +739,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     p.n_lines = g.voxels / g.M[2];
     p.n_tiles = (p.n_lines + e->CC - 1) / e->CC;
     p.partials = c->partials; p.state = c->state; p.hist = c->hist_dev; p.reduce_mode = RED_RESIDUAL;
+    p.dref = c->split ? c->dref : nullptr;
     const double vb = 8.0 * (double)g.voxels;
     if (c->ndim == 1) {
         p.slot0 = 0; p.finish = 1;
@@ -679,6 +749,13 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
         return MBS_OK;
     }
     const int mask01 = (e0 ? 1 : 0) | (e1 ? 2 : 0);
+    const bool act_on = activation_effective(c);
+    if (act_on) {
+        // before the update, activate the inactive subdomains whose transferred norm reached the threshold
+        KernelScope ks(c, "activation_step", 0.0);
+        MBS_CUDA(c, launch_activation_step(g, c->act, x, c->Kh_dev, to_cf(c->c), c->state, c->stream));
+        p.active = c->act.flags;
+    }
     if (mask01) MBS_TRY(run_slabs(c, x, nullptr, true, mask01));                      // corr_0(x), corr_1(x)
     if (c->use_line && e->line) {
         // warp-line sweeps: corr_2(x) inside sweep 1; corr_2(d) through the compact buffers like axes 0 and 1
@@ -741,6 +818,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
                 sp.ds = c->ds.buf[ax]; sp.u = c->u; sp.x = x; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
                 sp.e1 = e1; sp.e2 = e2; sp.alpha = (float)c->alpha; sp.partials = c->partials; sp.slot0 = slot;
                 sp.finish = (ax == last_ax) ? 1 : 0; sp.state = c->state; sp.hist = c->hist_dev;
+                sp.active = act_on ? c->act.flags : nullptr;
                 static const char* names[3] = {"slab_pass_ax0", "slab_pass_ax1", "slab_pass_ax2"};
                 KernelScope ks(c, names[ax], 40.0 * (double)corr_elems(g, ax));
                 MBS_CUDA(c, launch_slab_pass(g, sp, c->stream));
@@ -823,12 +901,61 @@ extern "C" int mbs_apply_operator(mbs_ctx* c, int which, const void* in_device, 
 // ---------------------------------------------------------------------------------------------
 // solve
 // ---------------------------------------------------------------------------------------------
+// ---------------------------------------------------------------------------------------------
+// Split iterate ("a compensated (hi + lo) x in the small, L2-resident configs").  The residual of Eq. (6),
+// r = B (x - (L+I)^-1 (B x + y_vec)), is a cancellation: the fp32 FFT of a field of size |x| leaves noise of about
+// 3e-7 |x| in it, a floor of (1-3)e-7 ||x|| / ||Gamma^-1 y|| under the relative residual (above config 1's tol of 1e-6).
+// Writing x = x_ref + delta with x_ref frozen, linearity gives
+//     x - (L+I)^-1 (B x + y_vec) = [x_ref - (L+I)^-1 (B x_ref + y_vec)] + [delta - (L+I)^-1 B delta] = d_ref + (delta - u'),
+// the same d as Eq. (6) in exact arithmetic, so the iteration, its residuals and its iteration count are unchanged; but
+// the FFT now acts on delta only and its rounding noise scales with |delta|, which shrinks as the iteration converges.
+// d_ref is computed once per re-centering (x_ref += delta, delta = 0), a few times per solve, when the residual has
+// dropped by two orders of magnitude.  Costs two extra arrays; the sweeps move the same bytes (the last sweep reads
+// d_ref, the first one reads no source).  Used on grids of <= 2^21 voxels (configs 1 and 2) unless MBS_OPT_REFINE says otherwise.
+// ---------------------------------------------------------------------------------------------
+static bool split_effective(const mbs_ctx* c) {
+    const bool want = c->refine == 1 || (c->refine < 0 && c->g.voxels <= (1LL << 21));
+    return want && c->fused && fused_available(c) && !c->use_merge && !c->activation;
+}
+
+static int recenter(mbs_ctx* c, const cf* y, cf* x, bool add_delta) {
+    const size_t bytes = sizeof(cf) * (size_t)c->g.voxels;
+    const double vb = 8.0 * (double)c->g.voxels;
+    if (add_delta) {                                          // x_ref <- x_ref + delta
+        PointwiseParams p = pw_defaults(c, false);
+        p.in = x; p.w = c->delta; p.s1 = 1.f; p.s2 = 1.f; p.out = x;
+        KernelScope ks(c, "recenter_add", 3 * vb);
+        MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
+    }
+    // u = (L+I)^-1 (B x_ref + y_vec)
+    MBS_TRY(run_B(c, x, nullptr, y, to_cf(-c->c), c->u, 1.f, nullptr, 0.f, RED_NONE, false));
+    MBS_TRY(run_propagator(c, c->u, 1, false));
+    {                                                         // d_ref = x_ref - u
+        PointwiseParams p = pw_defaults(c, false);
+        p.in = x; p.in2 = c->u; p.out = c->dref;
+        KernelScope ks(c, "recenter_dref", 3 * vb);
+        MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
+    }
+    {                                                         // ||x_ref||^2 -> DevState.xnorm2 (size of the rounding floor)
+        PointwiseParams p = pw_defaults(c, false);
+        p.in = x; p.reduce = RED_XNORM;
+        KernelScope ks(c, "recenter_norm", vb);
+        MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
+    }
+    MBS_CUDA(c, cudaMemsetAsync(c->delta, 0, bytes, c->stream));
+    c->n_recenter++;
+    return MBS_OK;
+}
+
 // Reset the device state for a new solve and (nu <= 0) compute nu = || B (L+I)^-1 y_vec ||
-static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, double nu) {
+static int begin_solve(mbs_ctx* c, const cf* y, const cf* x, double tol, int32_t max_iter, double nu) {
     c->u_ready = false;                               // the workspace u is scratch between solves
+    if (c->activation && !activation_effective(c))
+        return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation needs the default kernel options (fused warp-line sweeps, no merge)");
     DevState init{};
     init.iter = 0; init.done = 0; init.max_iter = max_iter; init.ticket = 0; init.tol = tol;
     init.nu2 = nu > 0 ? nu * nu : 0.0; init.last_sum = 0;
+    init.n_active = c->n_sub; init.n_sub = c->n_sub; init.xnorm2 = 0.0;
     c->state_pinned[0] = init;
     MBS_CUDA(c, cudaMemcpyAsync(c->state, &c->state_pinned[0], sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
     {
@@ -839,6 +966,25 @@ static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, do
         { KernelScope ks(c, "scale_copy", 16.0 * (double)c->g.voxels); MBS_CUDA(c, launch_scale_copy(y, c->u, to_cf(-c->c), c->g.voxels, c->stream)); }
         MBS_TRY(run_propagator(c, c->u, 1, false));
         MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
+    }
+    if (c->activation) {
+        // an inactive subdomain contributes d = 0: the compact d buffers must not hold values of an earlier solve
+        for (int ax = 0; ax < 3; ++ax)
+            if (c->ds.buf[ax]) MBS_CUDA(c, cudaMemsetAsync(c->ds.buf[ax], 0, sizeof(cf) * corr_elems(c->g, ax), c->stream));
+        const double thr = c->act_threshold >= 0 ? c->act_threshold : (tol > 0 ? 0.1 * tol : 0.0);
+        c->act.thr2 = thr * thr;
+        KernelScope ks(c, "activation_init", 16.0 * (double)c->g.voxels);
+        MBS_CUDA(c, launch_activation_init(c->g, c->act, y, x, c->state, c->stream));
+    }
+    c->split = false;
+    if (split_effective(c)) {
+        const size_t bytes = sizeof(cf) * (size_t)c->g.voxels;
+        if (!c->delta) { invalidate_graph(c); MBS_CUDA(c, cudaMalloc(&c->delta, bytes)); }
+        if (!c->dref) MBS_CUDA(c, cudaMalloc(&c->dref, bytes));
+        c->n_recenter = 0;
+        MBS_TRY(recenter(c, y, const_cast<cf*>(x), false));   // x_ref = x^(0), delta = 0
+        c->split = true;
+        c->split_eps = 1.0;
     }
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));   // state_pinned[0] is reused by the poll loop
     {
@@ -859,6 +1005,14 @@ static int begin_solve(mbs_ctx* c, const cf* y, double tol, int32_t max_iter, do
                         st.nu2 == 0 ? "the source y is identically zero: ||Gamma^-1 y|| = 0 and the relative residual is undefined"
                                     : "non-finite ||Gamma^-1 y||: the source or the medium holds NaN/Inf");
     }
+    return MBS_OK;
+}
+
+// iteration at which each subdomain was activated (all 0 when activation is off), for mbs_get_activation
+static int fetch_activation(mbs_ctx* c) {
+    c->act_iter_host.assign((size_t)c->n_sub, 0);
+    if (c->activation)
+        MBS_CUDA(c, cudaMemcpy(c->act_iter_host.data(), c->act.act_iter, sizeof(int32_t) * (size_t)c->n_sub, cudaMemcpyDeviceToHost));
     return MBS_OK;
 }
 
@@ -886,7 +1040,7 @@ static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_g
         for (int i = 0; i < batch; ++i) MBS_TRY(run_iteration(c, y, x));
         return MBS_OK;
     }
-    const bool stale = !c->graph_exec || c->graph_y != y || c->graph_x != x || c->graph_batch != batch ||
+    const bool stale = !c->graph_exec || c->graph_y != y || c->graph_x != x || c->graph_batch != batch || c->graph_split != (int)c->split ||
                        c->graph_fused != c->fused || c->graph_tma != c->use_tma || c->graph_line != c->use_line * 2 + c->use_merge;
     if (stale) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
@@ -907,7 +1061,7 @@ static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_g
         const cudaError_t e2 = cudaGraphInstantiate(&c->graph_exec, graph, 0);
         cudaGraphDestroy(graph);
         if (e2 != cudaSuccess) { c->graph_exec = nullptr; return fail(c, MBS_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e2)); }
-        c->graph_y = y; c->graph_x = x; c->graph_batch = batch;
+        c->graph_y = y; c->graph_x = x; c->graph_batch = batch; c->graph_split = (int)c->split;
         c->graph_fused = c->fused; c->graph_tma = c->use_tma; c->graph_line = c->use_line * 2 + c->use_merge;
         c->launches_per_batch = captured;
     }
@@ -922,15 +1076,16 @@ static int poll_interval(const mbs_ctx* c) {
     return (int)std::max<long long>(1, std::min<long long>(64, (64LL << 20) / std::max<long long>(1, c->g.voxels)));
 }
 
-static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_iter, double* residual_history,
+// The iteration loop behind mbs_solve, mbs_solve_host (stop test on: tol >= 0) and mbs_iterate (no stop test: tol < 0,
+// `nu` > 0 reuses a known normalisation).
+static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_iter, double nu, double* residual_history,
                         int32_t* n_iter) {
     if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
     if (!y || !x) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
     if (max_iter < 1) return fail(c, MBS_ERR_INVALID_ARG, "max_iter must be >= 1");
-    if (!(tol >= 0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0");
     if (n_iter) *n_iter = 0;
     MBS_TRY(ensure_history(c, max_iter));
-    MBS_TRY(begin_solve(c, y, tol, max_iter, 0.0));
+    MBS_TRY(begin_solve(c, y, x, tol, max_iter, nu));
 
     const int interval = poll_interval(c);
     MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
@@ -956,7 +1111,20 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
         if (pending[prev]) {
             MBS_CUDA(c, cudaEventSynchronize(c->ev_poll[prev]));
             pending[prev] = false;
-            if (c->state_pinned[prev].done) { final_done = c->state_pinned[prev].done; break; }
+            const DevState& st = c->state_pinned[prev];
+            if (st.done) { final_done = st.done; break; }
+            if (c->split && st.iter > 0 && st.nu2 > 0 && c->n_recenter < 16) {
+                // split iterate: re-centre each time the residual has dropped by an order of magnitude (what is enqueued
+                // here runs after the batch already in flight; in exact arithmetic it changes nothing).  A re-centring
+                // draws a fresh fp32 rounding of (L+I)^-1 (B x_ref + y_vec), a one-off perturbation of the size of the
+                // plain complex64 floor, about 2.4e-7 ||x|| / nu: it is done only while eps is 30 x above it.
+                const double eps = sqrt(st.last_sum / st.nu2);
+                const double floor_plain = 2.4e-7 * sqrt(st.xnorm2 / st.nu2);
+                if (eps < 0.1 * c->split_eps && eps > 30.0 * floor_plain) {
+                    MBS_TRY(recenter(c, y, x, true));
+                    c->split_eps = eps;
+                }
+            }
         }
         if (batch <= 0 || enqueued >= max_iter) {
             // nothing more to enqueue: drain the last poll
@@ -969,49 +1137,13 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
         }
         slot ^= 1;
     }
-    MBS_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
-    MBS_CUDA(c, cudaStreamSynchronize(c->stream));
-    DevState fin{};
-    MBS_CUDA(c, cudaMemcpy(&fin, c->state, sizeof(DevState), cudaMemcpyDeviceToHost));
-    float ms = 0.f;
-    MBS_CUDA(c, cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1));
-    c->last_solve_ms = ms;
-    prof_drain(c);
-    c->norm_rhs = sqrt(fin.nu2);
-    if (n_iter) *n_iter = fin.iter;
-    if (residual_history && fin.iter > 0)
-        MBS_CUDA(c, cudaMemcpy(residual_history, c->hist_dev, sizeof(double) * (size_t)fin.iter, cudaMemcpyDeviceToHost));
-    if (fin.done == 1) return MBS_OK;
-    if (fin.done == 3) return fail(c, MBS_ERR_NUMERIC, "non-finite residual at iteration %d", fin.iter - 1);
-    return fail(c, MBS_ERR_NOT_CONVERGED, "residual did not reach tol = %g within %d iterations", tol, max_iter);
-}
-
-extern "C" int mbs_solve(mbs_ctx* c, const void* y_device, void* x_device, double tol, int32_t max_iter,
-                         double* residual_history, int32_t* n_iter) {
-    if (!c) return MBS_ERR_INVALID_ARG;
-    return solve_device(c, (const cf*)y_device, (cf*)x_device, tol, max_iter, residual_history, n_iter);
-}
-
-extern "C" int mbs_iterate(mbs_ctx* c, const void* y_device, void* x_device, int32_t n_iter, double nu,
-                           double* residual_history) {
-    if (!c) return MBS_ERR_INVALID_ARG;
-    if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
-    if (!y_device || !x_device) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
-    if (n_iter < 1) return fail(c, MBS_ERR_INVALID_ARG, "n_iter must be >= 1");
-    MBS_TRY(ensure_history(c, n_iter));
-    MBS_TRY(begin_solve(c, (const cf*)y_device, -1.0, n_iter, nu));
-    MBS_CUDA(c, cudaEventRecord(c->ev_t0, c->stream));
-    {
-        // first batch launch by launch, the rest as graph replays of a full interval (kernels past n_iter return at
-        // once on the device flag), exactly as mbs_solve enqueues them
-        const int interval = poll_interval(c);
-        int enqueued = 0;
-        while (enqueued < n_iter) {
-            const bool first = (enqueued == 0);
-            const int batch = (first || !graphs_enabled(c)) ? std::min(interval, n_iter - enqueued) : interval;
-            MBS_TRY(enqueue_batch(c, (const cf*)y_device, (cf*)x_device, batch, !first));
-            enqueued += batch;
-        }
+    if (c->split) {
+        // x = x_ref + delta (kernels that were enqueued past the stop returned at once and left delta alone)
+        PointwiseParams p = pw_defaults(c, false);
+        p.in = x; p.w = c->delta; p.s1 = 1.f; p.s2 = 1.f; p.out = x;
+        KernelScope ks(c, "recenter_add", 24.0 * (double)c->g.voxels);
+        MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
+        c->split = false;
     }
     MBS_CUDA(c, cudaEventRecord(c->ev_t1, c->stream));
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -1020,12 +1152,30 @@ extern "C" int mbs_iterate(mbs_ctx* c, const void* y_device, void* x_device, int
     float ms = 0.f;
     MBS_CUDA(c, cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1));
     c->last_solve_ms = ms;
-    c->norm_rhs = sqrt(fin.nu2);
     prof_drain(c);
+    c->norm_rhs = sqrt(fin.nu2);
+    MBS_TRY(fetch_activation(c));
+    if (n_iter) *n_iter = fin.iter;
     if (residual_history && fin.iter > 0)
         MBS_CUDA(c, cudaMemcpy(residual_history, c->hist_dev, sizeof(double) * (size_t)fin.iter, cudaMemcpyDeviceToHost));
+    if (fin.done == 1) return MBS_OK;
     if (fin.done == 3) return fail(c, MBS_ERR_NUMERIC, "non-finite residual at iteration %d", fin.iter - 1);
-    return MBS_OK;
+    if (tol < 0) return MBS_OK;                       // mbs_iterate: exactly max_iter updates were asked for
+    return fail(c, MBS_ERR_NOT_CONVERGED, "residual did not reach tol = %g within %d iterations", tol, max_iter);
+}
+
+extern "C" int mbs_solve(mbs_ctx* c, const void* y_device, void* x_device, double tol, int32_t max_iter,
+                         double* residual_history, int32_t* n_iter) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (!(tol >= 0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0");
+    return solve_device(c, (const cf*)y_device, (cf*)x_device, tol, max_iter, 0.0, residual_history, n_iter);
+}
+
+extern "C" int mbs_iterate(mbs_ctx* c, const void* y_device, void* x_device, int32_t n_iter, double nu,
+                           double* residual_history) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (n_iter < 1) return fail(c, MBS_ERR_INVALID_ARG, "n_iter must be >= 1");
+    return solve_device(c, (const cf*)y_device, (cf*)x_device, -1.0, n_iter, nu, residual_history, nullptr);
 }
 
 extern "C" int mbs_get_kernel_stats(mbs_ctx* c, mbs_kernel_stat* out, int32_t capacity, int32_t* count) {
@@ -1062,7 +1212,8 @@ extern "C" int mbs_solve_host(mbs_ctx* c, const void* y_host, void* x_host, doub
     if (!c->host_x) MBS_CUDA(c, cudaMalloc(&c->host_x, bytes));
     MBS_CUDA(c, cudaMemcpyAsync(c->host_y, y_host, bytes, cudaMemcpyHostToDevice, c->stream));
     MBS_CUDA(c, cudaMemcpyAsync(c->host_x, x_host, bytes, cudaMemcpyHostToDevice, c->stream));
-    const int rc = solve_device(c, c->host_y, c->host_x, tol, max_iter, residual_history, n_iter);
+    if (!(tol >= 0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0");
+    const int rc = solve_device(c, c->host_y, c->host_x, tol, max_iter, 0.0, residual_history, n_iter);
     if (rc != MBS_OK && rc != MBS_ERR_NOT_CONVERGED) return rc;
     const std::string keep = c->err;
     MBS_CUDA(c, cudaMemcpyAsync(x_host, c->host_x, bytes, cudaMemcpyDeviceToHost, c->stream));

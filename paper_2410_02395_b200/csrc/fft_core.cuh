@@ -114,6 +114,14 @@ template <> struct Split<16> { static constexpr int A = 4, B = 4; };
 template <> struct Split<20> { static constexpr int A = 4, B = 5; };
 template <> struct Split<32> { static constexpr int A = 4, B = 8; };
 template <> struct Split<40> { static constexpr int A = 5, B = 8; };
+// radices of the 3^2 * 5 * 7 sizes (the paper's own 1260 = 2^2 3^2 5 7 voxels per axis)
+template <> struct Split<9>  { static constexpr int A = 3, B = 3; };
+template <> struct Split<14> { static constexpr int A = 2, B = 7; };
+template <> struct Split<15> { static constexpr int A = 3, B = 5; };
+template <> struct Split<18> { static constexpr int A = 2, B = 9; };
+template <> struct Split<21> { static constexpr int A = 3, B = 7; };
+template <> struct Split<30> { static constexpr int A = 5, B = 6; };
+template <> struct Split<42> { static constexpr int A = 6, B = 7; };
 
 template <int R, int BASE, int STRIDE, int P, class Enable = void>
 struct Dft;
@@ -183,6 +191,34 @@ struct Dft<5, BASE, STRIDE, P> {
     }
 };
 
+// radix 7: x_j +- x_{7-j} pairs; X_k = x0 + sum_j cos(2 pi jk/7) s_j -+ i sum_j sin(2 pi jk/7) d_j
+template <int BASE, int STRIDE, int P>
+struct Dft<7, BASE, STRIDE, P> {
+    static constexpr int slot(int k) { return k; }
+    static MBS_HD void run(cf (&v)[P]) {
+        constexpr float c1 = (float)cx_cos_2pi(1, 7), c2 = (float)cx_cos_2pi(2, 7), c3 = (float)cx_cos_2pi(3, 7);
+        constexpr float s1 = (float)cx_sin_2pi(1, 7), s2 = (float)cx_sin_2pi(2, 7), s3 = (float)cx_sin_2pi(3, 7);
+        const cf x0 = v[BASE];
+        const cf p1 = cadd(v[BASE + STRIDE], v[BASE + 6 * STRIDE]), m1 = csub(v[BASE + STRIDE], v[BASE + 6 * STRIDE]);
+        const cf p2 = cadd(v[BASE + 2 * STRIDE], v[BASE + 5 * STRIDE]), m2 = csub(v[BASE + 2 * STRIDE], v[BASE + 5 * STRIDE]);
+        const cf p3 = cadd(v[BASE + 3 * STRIDE], v[BASE + 4 * STRIDE]), m3 = csub(v[BASE + 3 * STRIDE], v[BASE + 4 * STRIDE]);
+        // k = 1: cos(1,2,3), sin(1,2,3);  k = 2: cos(2,4->3,6->1), sin(2, -3, -1);  k = 3: cos(3,6->1,9->2), sin(3, -1, 2)
+        const cf a1 = make_float2(x0.x + c1 * p1.x + c2 * p2.x + c3 * p3.x, x0.y + c1 * p1.y + c2 * p2.y + c3 * p3.y);
+        const cf a2 = make_float2(x0.x + c2 * p1.x + c3 * p2.x + c1 * p3.x, x0.y + c2 * p1.y + c3 * p2.y + c1 * p3.y);
+        const cf a3 = make_float2(x0.x + c3 * p1.x + c1 * p2.x + c2 * p3.x, x0.y + c3 * p1.y + c1 * p2.y + c2 * p3.y);
+        const cf b1 = make_float2(s1 * m1.x + s2 * m2.x + s3 * m3.x, s1 * m1.y + s2 * m2.y + s3 * m3.y);
+        const cf b2 = make_float2(s2 * m1.x - s3 * m2.x - s1 * m3.x, s2 * m1.y - s3 * m2.y - s1 * m3.y);
+        const cf b3 = make_float2(s3 * m1.x - s1 * m2.x + s2 * m3.x, s3 * m1.y - s1 * m2.y + s2 * m3.y);
+        v[BASE] = make_float2(x0.x + p1.x + p2.x + p3.x, x0.y + p1.y + p2.y + p3.y);
+        v[BASE + STRIDE] = make_float2(a1.x + b1.y, a1.y - b1.x);       // a - i b
+        v[BASE + 6 * STRIDE] = make_float2(a1.x - b1.y, a1.y + b1.x);   // a + i b
+        v[BASE + 2 * STRIDE] = make_float2(a2.x + b2.y, a2.y - b2.x);
+        v[BASE + 5 * STRIDE] = make_float2(a2.x - b2.y, a2.y + b2.x);
+        v[BASE + 3 * STRIDE] = make_float2(a3.x + b3.y, a3.y - b3.x);
+        v[BASE + 4 * STRIDE] = make_float2(a3.x - b3.y, a3.y + b3.x);
+    }
+};
+
 // composite R = A*B: n = B*n1 + n2, k = k1 + A*k2.
 //  step 1: for each n2, A-point DFT over n1 on slots B*n1 + n2      -> k1 at slot B*slotA(k1) + n2
 //  step 2: multiply (k1, n2) by W_R^{n2 k1}
@@ -238,13 +274,104 @@ struct Plan {
         return n == M_ && M_ % P_ == 0;
     }
     static_assert(valid(), "bad FFT plan");
+    static constexpr bool generic = false;
 };
+
+// Generic mixed-radix plan: the pass radices need not divide P (sizes with several odd prime factors, e.g.
+// 630 = 21 * 30).  The interface to the kernels is unchanged -- thread jt holds points jt + m*T, m < P, before and
+// after the transform -- but every pass goes through the shared-memory tile: pass i has M / R_i butterflies, thread jt
+// takes butterflies jt, jt + T, ... (the last round may be partial).
+template <int M_, int P_, int... Rs>
+struct GPlan {
+    static constexpr int M = M_;
+    static constexpr int P = P_;
+    static constexpr int T = M_ / P_;
+    static constexpr int NPASS = sizeof...(Rs) + 1;     // +1: kernels size their tiles by "more than one pass"
+    static constexpr int NR = sizeof...(Rs);
+    static constexpr int radix(int i) {
+        constexpr int r[sizeof...(Rs)] = {Rs...};
+        return r[i];
+    }
+    static constexpr int ns(int i) {
+        int n = 1;
+        for (int q = 0; q < i; ++q) n *= radix(q);
+        return n;
+    }
+    static constexpr bool valid() {
+        int n = 1;
+        for (int q = 0; q < NR; ++q) n *= radix(q);
+        return n == M_ && M_ % P_ == 0;
+    }
+    static_assert(valid(), "bad generic FFT plan");
+    static constexpr bool generic = true;
+};
+
+template <class PL, int SP, int SC>
+MBS_DEV void fft_line_forward_generic(cf (&v)[PL::P], cf* tile, const int c, const int jt, const cf* MBS_RESTRICT tw) {
+    constexpr int M = PL::M, P = PL::P, T = PL::T;
+    // natural order into the tile (the caller's v may differ from what the tile holds)
+    static_for<0, P>([&](auto mc) {
+        constexpr int m = decltype(mc)::value;
+        tile[(jt + m * T) * SP + c * SC] = v[m];
+    });
+    MBS_SYNC();
+    static_for<0, PL::NR>([&](auto ic) {
+        constexpr int i = decltype(ic)::value;
+        constexpr int R = PL::radix(i);
+        constexpr int Ns = PL::ns(i);
+        constexpr int NBF = M / R;                    // butterflies of this pass
+        constexpr int ROUNDS = (NBF + T - 1) / T;
+        cf w[ROUNDS][R];
+        static_for<0, ROUNDS>([&](auto qc) {
+            constexpr int q = decltype(qc)::value;
+            const int j = jt + q * T;
+            if (ROUNDS * T == NBF || j < NBF) {
+                static_for<0, R>([&](auto rc) {
+                    constexpr int r = decltype(rc)::value;
+                    w[q][r] = tile[(j + r * NBF) * SP + c * SC];
+                });
+                if constexpr (i > 0) {
+                    const int k = j % Ns;
+                    const int step = k * (M / (Ns * R));
+                    static_for<1, R>([&](auto rc) {
+                        constexpr int r = decltype(rc)::value;
+                        w[q][r] = cmul(w[q][r], tw[r * step]);
+                    });
+                }
+                Dft<R, 0, 1, R>::run(w[q]);
+            }
+        });
+        MBS_SYNC();                                   // every input of the pass has been read
+        static_for<0, ROUNDS>([&](auto qc) {
+            constexpr int q = decltype(qc)::value;
+            const int j = jt + q * T;
+            if (ROUNDS * T == NBF || j < NBF) {
+                const int k = j % Ns;
+                const int j0 = (j - k) * R + k;
+                static_for<0, R>([&](auto rc) {
+                    constexpr int r = decltype(rc)::value;
+                    tile[(j0 + r * Ns) * SP + c * SC] = w[q][Dft<R, 0, 1, R>::slot(r)];
+                });
+            }
+        });
+        MBS_SYNC();
+    });
+    static_for<0, P>([&](auto mc) {
+        constexpr int m = decltype(mc)::value;
+        v[m] = tile[(jt + m * T) * SP + c * SC];
+    });
+    MBS_SYNC();                                       // the tile is free again when the call returns
+}
 
 // One forward FFT of the line owned by (c, jt).  tile: shared memory, element (p, c) at
 // tile[p*SP + c*SC].  tw: table W_M^n = exp(-2 pi i n/M), n in [0, M) (shared or global).
 template <class PL, int SP, int SC>
 MBS_DEV void fft_line_forward(cf (&v)[PL::P], cf* tile, const int c, const int jt, const cf* MBS_RESTRICT tw) {
     constexpr int M = PL::M, P = PL::P, T = PL::T;
+    if constexpr (PL::generic) {
+        fft_line_forward_generic<PL, SP, SC>(v, tile, c, jt, tw);
+        return;
+    } else
     static_for<0, PL::NPASS>([&](auto ic) {
         constexpr int i = decltype(ic)::value;
         constexpr int R = PL::radix(i);

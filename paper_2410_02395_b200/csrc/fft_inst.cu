@@ -85,12 +85,14 @@ __global__ void __launch_bounds__(NTC) k_fft_contig(const cf* src, cf* dst, cons
     fft_contig_body<PL, CC, MODE>(src, dst, g, sp, tw, threadIdx.x, blockIdx.x, gridDim.x, reinterpret_cast<cf*>(smem_raw));
 }
 
+// the fused tile kernels move lines as pairs of voxels (128-bit accesses): odd subdomain lengths (63, 315) run unfused
+constexpr bool fused_ok() { return PL::M % 2 == 0; }
 template <int MODE>
 __global__ void __launch_bounds__(NTC) k_fused(const FusedParams p, const cf* __restrict__ tw, const int* __restrict__ done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     if (done && *done) return;
-    fused_contig_body<PL, CC, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
+    if constexpr (fused_ok()) fused_contig_body<PL, CC, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
 }
 
 // warp-line variant of the first / last sweep (line_kernels.cuh): 8 warps per CTA, each warp owns whole lines
@@ -390,7 +392,8 @@ cudaError_t contig_entry(const cf* src, cf* dst, const ContigGeom& g, const Symb
 #define MBS_CAT2(a, b) a##b
 #define MBS_CAT(a, b) MBS_CAT2(a, b)
 extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {
-    MBS_FFT_SIZE, CS, CSM, CC, strided_entry, contig_entry, fused_entry, fused_blocks_entry,
+    MBS_FFT_SIZE, CS, CSM, CC, strided_entry, contig_entry, fused_ok() ? fused_entry : nullptr,
+    fused_ok() ? fused_blocks_entry : nullptr,
     line_ok() ? line_entry : nullptr, line_ok() ? line_blocks_entry : nullptr,
     line_ok() ? merged_entry : nullptr, line_ok() ? merged_blocks_entry : nullptr};
 

@@ -55,7 +55,43 @@ struct StridedGeom {
     int inner;               // contiguous extent (product of the axes after)
     int tiles_inner;         // ceil(inner / C)
     long long n_tiles;       // n_outer * n_seg * tiles_inner
+    // subdomain activation: when act_list != nullptr the sweep visits only the tiles of the *n_act
+    // subdomains listed there (index (s0*S1 + s1)*S2 + s2); tile k of a listed subdomain, k in [0, tiles_per_sub):
+    //   sweep along axis 1:  outer = s0*M0 + k / tps2,              segment = s1, inner tile = s2*tps2 + k % tps2
+    //   sweep along axis 0:  segment = s0, i1 = s1*M1 + k / tps2,   inner tile = i1*(N2/C) + s2*tps2 + k % tps2
+    // with tps2 = M2 / C tiles per subdomain row (the host enables this only when C divides M2).
+    const int* act_list;
+    const int* n_act;
+    int axis;                // 0 or 1: the transformed axis in the internal 3-D description
+    int tiles_per_sub, tps2;
+    int S1, S2, M0, M1;      // subdomain counts of axes 1, 2; subdomain lengths of axes 0, 1
+    int row_tiles;           // N2 / C
 };
+
+// tile index -> (outer index, segment along the axis, inner tile) of a strided sweep
+MBS_HD void strided_tile_decode(const StridedGeom& g, const unsigned tix, unsigned& o, unsigned& seg, unsigned& ic) {
+    if (g.act_list) {
+        const unsigned u = tix / (unsigned)g.tiles_per_sub, k = tix - u * (unsigned)g.tiles_per_sub;
+        const unsigned sub = (unsigned)g.act_list[u];
+        const unsigned s2 = sub % (unsigned)g.S2, s01 = sub / (unsigned)g.S2;
+        const unsigned s1 = s01 % (unsigned)g.S1, s0 = s01 / (unsigned)g.S1;
+        const unsigned kr = k / (unsigned)g.tps2, kc = k - kr * (unsigned)g.tps2;
+        if (g.axis == 1) {
+            o = s0 * (unsigned)g.M0 + kr;
+            seg = s1;
+            ic = s2 * (unsigned)g.tps2 + kc;
+        } else {
+            o = 0;
+            seg = s0;
+            ic = (s1 * (unsigned)g.M1 + kr) * (unsigned)g.row_tiles + s2 * (unsigned)g.tps2 + kc;
+        }
+    } else {
+        const unsigned os = tix / (unsigned)g.tiles_inner;
+        ic = tix - os * (unsigned)g.tiles_inner;
+        o = os / (unsigned)g.n_seg;
+        seg = os - o * (unsigned)g.n_seg;
+    }
+}
 
 template <class PL, int C, int MODE>
 MBS_DEV void fft_strided_body(cf* MBS_RESTRICT data, const StridedGeom g, const SymbolParams sp,
@@ -68,11 +104,12 @@ MBS_DEV void fft_strided_body(cf* MBS_RESTRICT data, const StridedGeom g, const 
     MBS_SYNC();
     const int c = tid % C;
     const int jt = tid / C;
-    for (long long tix = bid; tix < g.n_tiles; tix += nblocks) {
-        const int ic = (int)(tix % g.tiles_inner);
-        const long long os = tix / g.tiles_inner;
-        const int s = (int)(os % g.n_seg);
-        const long long o = os / g.n_seg;
+    const long long n_tiles = g.act_list ? (long long)*g.n_act * g.tiles_per_sub : g.n_tiles;
+    for (long long tix = bid; tix < n_tiles; tix += nblocks) {
+        unsigned o_u, s_u, ic_u;
+        strided_tile_decode(g, (unsigned)tix, o_u, s_u, ic_u);
+        const int ic = (int)ic_u, s = (int)s_u;
+        const long long o = (long long)o_u;
         const int ii = ic * C + c;
         const bool valid = ii < g.inner;
         cf* base = data + o * g.outer_stride + (long long)s * M * g.stride + ii;

@@ -91,17 +91,16 @@ __device__ __forceinline__ void fft_strided_tma_body(const CUtensorMap* map, con
     const int c = tid % C;
     const int jt = tid / C;
     // tile counters fit 32 bits (fewer than 2^31 voxels): keep the per-tile index arithmetic cheap
-    const unsigned first = blockIdx.x, step = gridDim.x, n_tiles = (unsigned)g.n_tiles;
+    const unsigned first = blockIdx.x, step = gridDim.x;
+    // with subdomain activation the sweep covers the listed subdomains only (the count lives in device memory)
+    const unsigned n_tiles = g.act_list ? (unsigned)*g.n_act * (unsigned)g.tiles_per_sub : (unsigned)g.n_tiles;
     const unsigned n_mine = first < n_tiles ? (n_tiles - first + step - 1) / step : 0;
-    const unsigned tiles_inner = (unsigned)g.tiles_inner, n_seg = (unsigned)g.n_seg;
 
     auto coords = [&](unsigned i, int& c0, int& c1, int& c2, int& ii0) {
-        const unsigned tix = first + i * step;
-        const unsigned os = tix / tiles_inner;
-        const unsigned ic = tix - os * tiles_inner;
-        const unsigned o = os / n_seg;
+        unsigned o, seg, ic;
+        strided_tile_decode(g, first + i * step, o, seg, ic);
         c0 = (int)(2 * ic * C);
-        c1 = (int)(os - o * n_seg) * M;
+        c1 = (int)seg * M;
         c2 = (int)o;
         ii0 = (int)(ic * C);
     };

@@ -134,7 +134,12 @@ __device__ __forceinline__ float fused_epi_line(const FusedParams& p, const cf* 
         const int q = 2 * lane + 64 * k;
         if (M % 64 == 0 || q < M) {
             const cf2 xv = ld2(xl + q), bv = ld2(bl + q);
-            const cf d0 = csub(xv.a, trow[q]), d1 = csub(xv.b, trow[q + 1]);
+            cf d0 = csub(xv.a, trow[q]), d1 = csub(xv.b, trow[q + 1]);
+            if (p.dref) {                                     // split iterate: d = d_ref + (delta - u')
+                const cf2 dv = ld2(p.dref + gl + q);
+                d0 = cadd(d0, dv.a);
+                d1 = cadd(d1, dv.b);
+            }
             cf r0 = cmul(bv.a, d0), r1 = cmul(bv.b, d1);
             if (p.a2 && (64 * k < t || 64 * k + 64 > M - t)) {
                 if (q < t) r0 = csub(r0, cel[q]);
@@ -283,7 +288,9 @@ __device__ __forceinline__ void fused_contig_body(const FusedParams& p, const cf
                 for (int o = tid; o < nvalid * t2; o += NT) {
                     const int line = o / t2, e = o - line * t2;
                     const int q = (e < t ? e : M - t2 + e);
-                    ed[o] = csub(p.x[g0 + (long long)line * M + q], tile[line * LS + q]);
+                    cf dv = csub(p.x[g0 + (long long)line * M + q], tile[line * LS + q]);
+                    if (p.dref) dv = cadd(dv, p.dref[g0 + (long long)line * M + q]);
+                    ed[o] = dv;
                 }
                 __syncthreads();
                 fused_corr2<C>(ed, ce, Ks, t, p.S2, p.per2, p.c, nvalid, tid, NT);

@@ -291,6 +291,14 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
             if (g.per[ax]) nb = (nb + S) % S;
             else has_nb = false;
         }
+        if (p.active) {
+            // subdomain activation: the edge voxels of an inactive subdomain are left alone
+            int s0, s1, s2;
+            if (ax == 0) { s0 = s; s1 = (int)(in_i / g.N[2]) / g.M[1]; s2 = (int)(in_i % g.N[2]) / g.M[2]; }
+            else if (ax == 1) { s0 = (int)o / g.M[0]; s1 = s; s2 = (int)in_i / g.M[2]; }
+            else { s0 = (int)(o / g.N[1]) / g.M[0]; s1 = (int)(o % g.N[1]) / g.M[1]; s2 = s; }
+            if (!p.active[(s0 * g.S[1] + s1) * g.S[2] + s2]) continue;
+        }
         // side 1 (last t points of s) reads the FIRST t points of s and s+1; side 0 reads the LAST t points
         const long long own0 = ((o * S + s) * 2 * t + (side ? 0 : t)) * inner + in_i;
         const long long nb0 = ((o * S + nb) * 2 * t + (side ? 0 : t)) * inner + in_i;
@@ -641,6 +649,170 @@ cudaError_t launch_scale_copy(const cf* in, cf* out, cf scale, long long n, cuda
     long long nb = (n + 255) / 256;
     if (nb > 148 * 32) nb = 148 * 32;
     k_scale_copy<<<(unsigned)nb, 256, 0, st>>>(in, out, scale, n);
+    return cudaGetLastError();
+}
+
+// ---------------------------------------------------------------------------------------------
+// Subdomain activation ("initially activating only those subdomains that hold a source term.  Neighbouring
+// subdomains are activated only after the norm of the transferred field exceeds a certain threshold"; reading R17).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ int subdomain_of(const GridDesc& g, int i0, int i1, int i2) {
+    return ((i0 / g.M[0]) * g.S[1] + i1 / g.M[1]) * g.S[2] + i2 / g.M[2];
+}
+
+// flags[s] = 1 if y or x is non-zero anywhere in subdomain s (flags are zeroed before the launch)
+__global__ void __launch_bounds__(256) k_activation_mark(const GridDesc g, const cf* __restrict__ y, const cf* __restrict__ x,
+                                                         int* __restrict__ flags) {
+    const long long rows = g.voxels / g.N[2];
+    const int lane = threadIdx.x & 31;
+    const long long warp0 = ((long long)blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+    const long long nwarps = ((long long)gridDim.x * blockDim.x) >> 5;
+    for (long long row = warp0; row < rows; row += nwarps) {
+        const int i1 = (int)(row % g.N[1]), i0 = (int)(row / g.N[1]);
+        const cf* yr = y + row * g.N[2];
+        const cf* xr = x + row * g.N[2];
+        for (int s2 = 0; s2 < g.S[2]; ++s2) {
+            bool nz = false;
+            for (int i = s2 * g.M[2] + lane; i < (s2 + 1) * g.M[2]; i += 32) {
+                const cf a = yr[i], b = xr[i];
+                nz = nz || a.x != 0.f || a.y != 0.f || b.x != 0.f || b.y != 0.f;
+            }
+            if (__any_sync(0xffffffffu, nz) && lane == 0) flags[subdomain_of(g, i0, i1, s2 * g.M[2])] = 1;
+        }
+    }
+}
+
+// list of the active subdomains in ascending order, their number, and the activation iteration of the initial set
+__global__ void k_activation_list(const int n_sub, int* flags, int* list, int* n_act, int* act_iter, DevState* state,
+                                  const int init) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    int n = 0;
+    for (int s = 0; s < n_sub; ++s) {
+        if (init) act_iter[s] = flags[s] ? 0 : -1;
+        if (flags[s]) list[n++] = s;
+    }
+    *n_act = n;
+    state->n_active = n;
+    state->n_sub = n_sub;
+}
+
+// One block per (subdomain s, face f = axis*2 + side, chunk): partial sum of |corr_axis(x)|^2 over the t edge points of
+// that face of an INACTIVE s whose neighbour across the face is ACTIVE (x_s = 0, so corr is what the neighbour transfers):
+//   side 0 (first t points of s):  corr[b] = c sum_a Kh[a][b] x_{s-1}[M-t+a]
+//   side 1 (last  t points of s):  corr[a] = c sum_b Kh[a][b] x_{s+1}[b]            (kernels above)
+// The last block to finish adds the partials per subdomain in a fixed order, activates s when
+// T_s^2 >= thr2 * nu^2, and rebuilds the list.
+template <int TT>
+__global__ void __launch_bounds__(256) k_activation_step(const GridDesc g, const ActivationState a, const cf* __restrict__ x,
+                                                         const float* __restrict__ Kh, const cf c, DevState* state) {
+    __shared__ float Ks[TT * TT];
+    __shared__ double red[32];
+    __shared__ int s_last;
+    if (state->done) return;
+    const int n_sub = g.S[0] * g.S[1] * g.S[2];
+    if (*a.n_act == n_sub) return;                    // everything is active: nothing to decide
+    const int t = TT;
+    for (int i = threadIdx.x; i < TT * TT; i += blockDim.x) Ks[i] = Kh[i];
+    __syncthreads();
+    const int ch = blockIdx.x % ACT_CHUNKS;
+    const int f = (blockIdx.x / ACT_CHUNKS) % 6;
+    const int s = blockIdx.x / (ACT_CHUNKS * 6);
+    const int ax = f >> 1, side = f & 1;
+    int sd[3];
+    sd[2] = s % g.S[2]; sd[1] = (s / g.S[2]) % g.S[1]; sd[0] = s / (g.S[2] * g.S[1]);
+    float acc = 0.f;
+    bool live = a.flags[s] == 0 && g.a[ax] > 0;
+    int nbd[3] = {sd[0], sd[1], sd[2]};
+    if (live) {
+        int nb = side ? sd[ax] + 1 : sd[ax] - 1;
+        if (nb < 0 || nb >= g.S[ax]) {
+            if (g.per[ax] && g.S[ax] > 1) nb = (nb + g.S[ax]) % g.S[ax];
+            else live = false;
+        }
+        nbd[ax] = nb;
+        if (live) live = a.flags[(nbd[0] * g.S[1] + nbd[1]) * g.S[2] + nbd[2]] != 0;
+    }
+    if (live) {
+        const int d1 = ax == 0 ? 1 : 0, d2 = ax == 2 ? 1 : 2;   // the two transverse axes, d2 the faster one
+        const long long stride[3] = {(long long)g.N[1] * g.N[2], (long long)g.N[2], 1LL};
+        const int n1 = g.M[d1], n2 = g.M[d2];
+        const int n_items = n1 * n2;
+        const int per_chunk = (n_items + ACT_CHUNKS - 1) / ACT_CHUNKS;
+        const int lo = ch * per_chunk, hi = min(n_items, lo + per_chunk);
+        // first point read along the axis: the neighbour's LAST t points (side 0) or FIRST t points (side 1)
+        const long long base = ((long long)nbd[ax] * g.M[ax] + (side ? 0 : g.M[ax] - t)) * stride[ax] +
+                               (long long)sd[d1] * g.M[d1] * stride[d1] + (long long)sd[d2] * g.M[d2] * stride[d2];
+        for (int item = lo + (int)threadIdx.x; item < hi; item += (int)blockDim.x) {
+            const int j1 = item / n2, j2 = item - j1 * n2;
+            const cf* src = x + base + j1 * stride[d1] + j2 * stride[d2];
+            cf v[TT];
+#pragma unroll
+            for (int q = 0; q < TT; ++q) v[q] = src[q * stride[ax]];
+#pragma unroll
+            for (int e = 0; e < TT; ++e) {
+                float sr = 0.f, si = 0.f;
+#pragma unroll
+                for (int q = 0; q < TT; ++q) {
+                    const float k = side ? Ks[e * TT + q] : Ks[q * TT + e];
+                    sr = fmaf(k, v[q].x, sr);
+                    si = fmaf(k, v[q].y, si);
+                }
+                const cf cc = cmul(c, make_float2(sr, si));
+                acc += cc.x * cc.x + cc.y * cc.y;
+            }
+        }
+    }
+    const double bs = block_sum((double)acc, red);
+    if (threadIdx.x == 0) {
+        a.partials[blockIdx.x] = bs;
+        __threadfence();
+        s_last = (atomicAdd(a.ticket, 1u) == gridDim.x - 1);
+    }
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int q = threadIdx.x; q < n_sub; q += blockDim.x) {
+        if (a.flags[q]) continue;
+        double T2 = 0.0;
+        for (int i = 0; i < 6 * ACT_CHUNKS; ++i) T2 += __ldcg(&a.partials[q * 6 * ACT_CHUNKS + i]);
+        if (T2 >= a.thr2 * state->nu2) {
+            a.flags[q] = 1;
+            a.act_iter[q] = state->iter;
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        *a.ticket = 0;
+        int n = 0;
+        for (int q = 0; q < n_sub; ++q)
+            if (a.flags[q]) a.list[n++] = q;
+        *a.n_act = n;
+        state->n_active = n;
+    }
+}
+
+cudaError_t launch_activation_init(const GridDesc& g, const ActivationState& a, const cf* y, const cf* x, DevState* state,
+                                   cudaStream_t st) {
+    const int n_sub = g.S[0] * g.S[1] * g.S[2];
+    cudaError_t e = cudaMemsetAsync(a.flags, 0, sizeof(int) * n_sub, st);
+    if (e != cudaSuccess) return e;
+    if ((e = cudaMemsetAsync(a.ticket, 0, sizeof(unsigned int), st)) != cudaSuccess) return e;
+    k_activation_mark<<<148 * 8, 256, 0, st>>>(g, y, x, a.flags);
+    k_activation_list<<<1, 32, 0, st>>>(n_sub, a.flags, a.list, a.n_act, a.act_iter, state, 1);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_activation_step(const GridDesc& g, const ActivationState& a, const cf* x, const float* Kh, cf c,
+                                   DevState* state, cudaStream_t st) {
+    const int n_sub = g.S[0] * g.S[1] * g.S[2];
+    const unsigned nb = (unsigned)(n_sub * 6 * ACT_CHUNKS);
+    switch (g.t) {
+        case 2: k_activation_step<2><<<nb, 256, 0, st>>>(g, a, x, Kh, c, state); break;
+        case 4: k_activation_step<4><<<nb, 256, 0, st>>>(g, a, x, Kh, c, state); break;
+        case 8: k_activation_step<8><<<nb, 256, 0, st>>>(g, a, x, Kh, c, state); break;
+        case 16: k_activation_step<16><<<nb, 256, 0, st>>>(g, a, x, Kh, c, state); break;
+        default: return cudaErrorNotSupported;
+    }
     return cudaGetLastError();
 }
 

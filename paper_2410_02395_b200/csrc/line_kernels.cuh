@@ -156,7 +156,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
     float acc = 0.f;
     for (unsigned unit = blockIdx.x * NWARP + warp; unit < n_units; unit += gridDim.x * NWARP) {
         unsigned line = unit * LW + lsub;
-        const bool valid = line < n_lines;
+        bool valid = line < n_lines;
         unsigned row = line / (unsigned)p.S2;
         const int seg = (int)(line - row * (unsigned)p.S2);
         if (MODE == LINE_S1 && p.slab_rows_only) {    // `line` counted slab-row lines: map to the real row
@@ -164,6 +164,11 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
             line = row * (unsigned)p.S2 + (unsigned)seg;
         }
         const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
+        if (p.active) {
+            // subdomain activation: the lines of an inactive subdomain are not computed
+            if (valid) valid = p.active[((i0 / p.M0) * p.S1 + i1 / p.M1) * p.S2 + seg] != 0;
+            if (!__any_sync(0xffffffffu, valid)) continue;
+        }
         long long o0 = -1, o1 = -1;                   // compact row offsets of the axis-0 / axis-1 slabs
         if (valid && p.e0) {
             const int q = line_edge_slot(i0, p.M0, t);
@@ -213,7 +218,13 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
             // request: no registers, no shared memory), so that their loads after this FFT are L2 hits
             if (!p.slab_rows_only) {
                 const unsigned nline = (unit + gridDim.x * NWARP) * LW + lsub;
-                if (nline < n_lines) {
+                bool want = nline < n_lines;
+                if (want && p.active) {
+                    const unsigned nrow = nline / (unsigned)p.S2;
+                    const int ni0 = (int)(nrow / (unsigned)p.N1), ni1 = (int)(nrow - (unsigned)ni0 * (unsigned)p.N1);
+                    want = p.active[((ni0 / p.M0) * p.S1 + ni1 / p.M1) * p.S2 + (int)(nline - nrow * (unsigned)p.S2)] != 0;
+                }
+                if (want) {
                     const char* nx = reinterpret_cast<const char*>(p.x + (long long)nline * M);
                     const char* nb = reinterpret_cast<const char*>(p.bdiag + (long long)nline * M);
                     for (int off = jt * 128; off < M * (int)sizeof(cf); off += T * 128) {
@@ -264,7 +275,8 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                     constexpr int m = decltype(mc)::value;
                     const int pidx = jt + m * T;
                     const cf xv = xr[m];
-                    const cf d = csub(xv, cswap(v[m]));
+                    cf d = csub(xv, cswap(v[m]));
+                    if (p.dref) d = cadd(d, p.dref[gl + pidx]);        // split iterate: d = d_ref + (delta - u')
                     cf bv;
                     if constexpr (PREFETCH_B) bv = br[m];
                     else bv = bst[pidx];

@@ -42,9 +42,12 @@ struct DevState {
     double tol;
     double nu2;             // ||Gamma^-1 y_vec||^2
     double last_sum;        // last reduced sum (for norm queries)
+    int n_active;           // subdomain activation: active subdomains (= all of them when it is off)
+    int n_sub;
+    double xnorm2;          // ||x_ref||^2 at the last re-centering of the split iterate (api.cu recenter())
 };
 
-enum ReduceMode { RED_NONE = 0, RED_NU2 = 1, RED_RESIDUAL = 2, RED_PLAIN = 3 };
+enum ReduceMode { RED_NONE = 0, RED_NU2 = 1, RED_RESIDUAL = 2, RED_PLAIN = 3, RED_XNORM = 4 };
 
 // Pointwise pass:  val = B_diag*(in - in2) + ysc*y - corr;   (each term optional)
 //   update == 0:   out = s1*val + s2*w
@@ -118,6 +121,8 @@ struct SlabPassParams {
     int finish;        // 1: this is the last pass: add all partials [0, slot0 + grid) and finish the iteration
     DevState* state;
     double* hist;
+    const int* active; // subdomain activation: flags per subdomain (s0*S1 + s1)*S2 + s2, or nullptr (all active);
+                       // the edge voxels of an inactive subdomain are left alone (no update, no residual)
 };
 int slab_pass_blocks(const GridDesc& g, int ax);
 bool slab_pass_supported(int t);
@@ -175,7 +180,33 @@ struct FusedParams {
     int slot0, n_total, finish, reduce_mode;
     DevState* state;
     double* hist;
+    const int* active;   // subdomain activation: flags per subdomain, or nullptr; lines of an inactive
+                         // subdomain are skipped by the warp-line sweeps
+    const cf* dref;      // split iterate (api.cu "refinement"): the sweeps run on the small part delta of x = x_ref + delta,
+                         // and the last sweep adds d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec) to d = delta - u'; or nullptr
 };
+
+// Subdomain activation (reading R17 of DESIGN.md section 3).  Device-resident: flags[n_sub], the list of
+// the active subdomains in index order + its length (read by the strided sweeps), the iteration at which each
+// subdomain was activated, per-block partial sums of the transferred norms.
+struct ActivationState {
+    int* flags;          // [n_sub]
+    int* list;           // [n_sub] active subdomain indices, ascending
+    int* n_act;          // [1]
+    int* act_iter;       // [n_sub] iteration of activation, -1 = not yet
+    double* partials;    // [n_sub][6][ACT_CHUNKS]
+    unsigned int* ticket;
+    double thr2;         // threshold^2 (relative to nu^2)
+};
+constexpr int ACT_CHUNKS = 8;
+// flags from the source and the start vector (a subdomain is active from the start if y or x0 is non-zero in it)
+cudaError_t launch_activation_init(const GridDesc& g, const ActivationState& a, const cf* y, const cf* x, DevState* state,
+                                   cudaStream_t st);
+// before update n: T_s^2 = sum_d ||corr_d(x)_s||^2 for every inactive subdomain s (what its active neighbours
+// transfer into it); activates s when T_s^2 >= thr2 * nu^2; rebuilds the list.  Deterministic (fixed-order sums).
+cudaError_t launch_activation_step(const GridDesc& g, const ActivationState& a, const cf* x, const float* Kh, cf c,
+                                   DevState* state, cudaStream_t st);
+
 
 // FFT registry (fft_inst.cu compiled once per size, fft_registry.cu)
 struct FftEntry {

@@ -30,6 +30,7 @@ __device__ __forceinline__ double block_sum(double v, double* red) {
 //   RED_NU2       nu^2 = sum                                   (||Gamma^-1 y_vec||^2)
 //   RED_RESIDUAL  eps_n = sqrt(sum / nu^2) -> hist[n], n + 1 -> iter, stop flag (R7, R8)
 //   RED_PLAIN     last_sum = sum
+//   RED_XNORM     xnorm2 = sum (last_sum untouched: the host derives eps from it)
 // partials written by earlier launches on the same stream (slots below slot0) are included.
 __device__ __forceinline__ void grid_reduce_finish(double block_partial, double* partials, int slot0, int n_total,
                                                    int finish, int mode, DevState* s, double* hist, double* red) {
@@ -51,8 +52,10 @@ __device__ __forceinline__ void grid_reduce_finish(double block_partial, double*
     const double total = block_sum(acc, red);
     if (threadIdx.x == 0) {
         s->ticket = 0;
-        s->last_sum = total;
-        if (mode == RED_NU2) {
+        if (mode != RED_XNORM) s->last_sum = total;
+        if (mode == RED_XNORM) {
+            s->xnorm2 = total;
+        } else if (mode == RED_NU2) {
             s->nu2 = total;
         } else if (mode == RED_RESIDUAL) {
             const double eps = sqrt(total / s->nu2);

@@ -171,10 +171,37 @@ def _source_cfg5(w: Workload) -> np.ndarray:
     return y
 
 
+def _medium_paper_large(w: Workload) -> np.ndarray:
+    """Stand-in for the structure of the paper's large run (section 4.3): spheres of radius 6 wavelengths
+    (24 px), n = 1.33 with a small imaginary part, in n = 1, with a clearance of 6 wavelengths between them.  PoreSpy
+    is not available: the centres sit on a cubic lattice of pitch 2r + clearance = 72 px, each jittered by up to
+    +-10 px per axis and kept with probability 0.8 (seeded), which keeps a clearance of at least 4 px."""
+    rng = np.random.default_rng(w.seed)
+    pitch, rad = 72.0, 24.0
+    axes = [np.arange(pitch / 2, s, pitch) for s in w.shape]
+    grid = np.stack(np.meshgrid(*axes, indexing="ij"), axis=-1).reshape(-1, w.ndim)
+    grid = grid + rng.uniform(-10.0, 10.0, size=grid.shape)
+    keep = rng.uniform(size=len(grid)) < 0.8
+    centres = grid[keep]
+    n = np.ones(w.shape, dtype=np.complex64)
+    _paint_balls(n, centres, np.full(len(centres), rad), np.full(len(centres), 1.33 + 0.001j, dtype=np.complex64))
+    return n
+
+
+def _source_plane_near_face(w: Workload) -> np.ndarray:
+    """Planar source just inside the absorbing layer of the axis-0 face ("planar source located at x = 0", section 4)."""
+    y = np.zeros(w.shape, dtype=np.complex64)
+    y[w.boundary_width[0] + 4] = 1.0
+    return y
+
+
 def config(cfg: int, shape: Tuple[int, ...] = None, boundary_width: Tuple[int, ...] = None,
            tol: float = None, max_iter: int = None) -> Workload:
     """BASELINE.json config `cfg` (1..5).  `shape` overrides the grid for the reduced-size
-    parity stand-ins (same generator, same subdomain counts, object count scaled by volume)."""
+    parity stand-ins (same generator, same subdomain counts, object count scaled by volume).
+    cfg 6 is not a BASELINE.json config: it is the SHAPE of the paper's own large run (1260^3 voxels = 315^3
+    wavelengths, two subdomains along x, 5-wavelength absorbing layers; section 4.3, Table 1), with a
+    synthetic stand-in for its structure; bench.py quotes it as context beside the paper's numbers."""
     table = {
         1: dict(shape=(256,), S=(2,), W=(8,), tol=1e-6, max_iter=20000,
                 medium=_medium_cfg1, source=_source_cfg1),
@@ -186,6 +213,8 @@ def config(cfg: int, shape: Tuple[int, ...] = None, boundary_width: Tuple[int, .
                 medium=_medium_cfg4, source=_source_cfg4),
         5: dict(shape=(1024, 1024, 1024), S=(4, 2, 2), W=(32, 32, 32), tol=1e-3, max_iter=200000,
                 medium=_medium_cfg5, source=_source_cfg5),
+        6: dict(shape=(1260, 1260, 1260), S=(2, 1, 1), W=(20, 20, 20), tol=1e-3, max_iter=200000,
+                medium=_medium_paper_large, source=_source_plane_near_face),
     }
     e = table[cfg]
     shp = tuple(shape) if shape is not None else e["shape"]

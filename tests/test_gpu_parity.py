@@ -138,7 +138,33 @@ PLAN_CASES = [
     ((16, 16, 384), (1, 1, 1), (2, 2, 8), 8, None),
     ((128, 256, 32), (1, 1, 1), (4, 4, 4), 8, None),         # cfg 3's subdomain lengths on axes 0, 1
 ]
-OPERATOR_CASES = OPERATOR_CASES + PLAN_CASES
+# Sizes with the factors 3^2, 5^2 and 7 (NEXT-3 of SURVEY 8(f): the paper's own grid is 1260 = 2^2 3^2 5 7 voxels per axis,
+# P:195; its validation run is 200^3).  Generic two-pass plans (fft_core.cuh GPlan) through the tile kernels.
+ODD_SIZE_CASES = [
+    ((126, 63, 90), (1, 1, 1), (4, 4, 4), 8, None),          # 126 kernel-multiply, 63 strided, 90 contiguous
+    ((252, 16, 40), (1, 1, 1), (8, 2, 4), 8, None),
+    ((16, 252, 40), (1, 1, 1), (2, 8, 4), 8, None),
+    ((16, 16, 504), (1, 1, 2), (2, 2, 8), 8, None),          # 252 contiguous, two subdomains
+    ((315, 16, 40), (1, 1, 1), (8, 2, 4), 8, None),
+    ((16, 315, 40), (1, 1, 1), (2, 8, 4), 8, None),
+    ((16, 16, 630), (1, 1, 2), (2, 2, 8), 8, None),          # 315 contiguous, two subdomains
+    ((1260, 16, 40), (2, 1, 1), (8, 2, 4), 8, None),         # 630 kernel-multiply sweep, two subdomains (the paper's split)
+    ((16, 630, 40), (1, 1, 1), (2, 8, 4), 8, None),          # 630 strided: three TMA boxes of 210 rows
+    ((16, 16, 630), (1, 1, 1), (2, 2, 8), 8, None),
+    ((1260, 40), (1, 1), (16, 4), 8, None),                  # 1260: one domain along an axis (the paper's CPU run)
+    ((16, 1260, 16), (1, 1, 1), (2, 16, 2), 8, None),
+    ((16, 16, 1260), (1, 1, 1), (2, 2, 16), 8, None),
+    ((420, 40), (1, 1), (8, 4), 8, None),
+    ((16, 16, 1260), (1, 1, 3), (2, 2, 16), 8, None),        # 420 contiguous, three subdomains
+    ((360, 40), (1, 1), (8, 4), 8, None),
+    ((16, 180, 40), (1, 1, 1), (2, 8, 4), 8, None),
+    ((16, 16, 360), (1, 1, 1), (2, 2, 8), 8, None),
+    ((200, 40), (2, 1), (8, 4), 8, None),                    # 100
+    ((16, 200, 40), (1, 1, 1), (2, 8, 4), 8, None),
+    ((16, 16, 400), (1, 1, 1), (2, 2, 8), 8, None),
+    ((400, 16, 40), (1, 1, 1), (8, 2, 4), 8, None),
+]
+OPERATOR_CASES = OPERATOR_CASES + PLAN_CASES + ODD_SIZE_CASES
 
 
 @pytest.mark.parametrize("shape,S,W,t,periodic", OPERATOR_CASES)
@@ -640,3 +666,47 @@ def test_graph_reuse_across_solves(B):
     assert np.array_equal(h4, h5) and torch.equal(x5, xd)
     s.close()
     s2.close()
+
+
+ACTIVATION_CASES = [
+    # name, workload, threshold (None = tol / 10, the default of R17)
+    ("cfg5_small", lambda: workloads.config(5, shape=(128, 64, 64), boundary_width=(8, 8, 8)), None),
+    ("cfg5_small_thr_tol", lambda: workloads.config(5, shape=(128, 64, 64), boundary_width=(8, 8, 8)), 1e-3),
+    ("cfg2_small", lambda: workloads.config(2, shape=(256, 256), boundary_width=(16, 16), tol=1e-3), None),
+    ("cfg3_small_4x1x1", lambda: dataclasses.replace(
+        workloads.config(3, shape=(256, 32, 32), boundary_width=(8, 8, 8)), n_subdomains=(4, 1, 1)), 1e-2),
+]
+
+
+@pytest.mark.parametrize("name,make,thr", ACTIVATION_CASES)
+def test_subdomain_activation_parity(B, orc, name, make, thr):
+    """Subdomain activation (reading R17): the CUDA path and the oracle's solve_activated follow the same
+    rule, so the subdomains are activated at the same iterations (+-1: the transferred norm is compared in fp32 /
+    fp64), the iteration counts agree +-1 and the fields agree to 1e-4; and the activated solve reaches the field of
+    the plain one ("converges to the correct solution from any starting point")."""
+    w = make()
+    n, y = w.make_medium(), w.make_source()
+    o = orc.from_workload(w, n)
+    x_ref, h_ref, act_ref = orc.solve_activated(o, y, tol=w.tol, max_iter=w.max_iter, threshold=thr)
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    x_plain, h_plain, rc = s.solve(y, tol=w.tol, max_iter=w.max_iter)
+    assert rc == B.MBS_OK and s.activation() == [0] * len(act_ref)
+    s.set_activation(True, -1.0 if thr is None else thr)
+    x, hist, rc = s.solve(y, tol=w.tol, max_iter=w.max_iter)
+    act = s.activation()
+    print("%s: activated at %s (oracle %s); iterations %d (oracle %d, plain %d)" % (name, act, act_ref, len(hist), len(h_ref), len(h_plain)))
+    assert rc == B.MBS_OK
+    assert any(a > 0 for a in act_ref), "the case must exercise activation"
+    assert len(act) == len(act_ref) and all(abs(a - b) <= 1 for a, b in zip(act, act_ref))
+    assert abs(len(hist) - len(h_ref)) <= 1
+    check_field(x.cpu().numpy(), x_ref, FIELD_TOL, w.shape, w.n_subdomains, w.n_correction, what=name)
+    assert np.allclose(hist[:5], h_ref[:5], rtol=1e-4)
+    # the same field as without activation, at the level of the stopping threshold
+    assert rel(x.cpu().numpy(), x_plain.cpu().numpy()) <= 3.0 * max(w.tol, 10 * (thr or 0.0))
+    # switching it off again restores the plain iteration bit for bit
+    s.set_activation(False)
+    x2, h2, rc2 = s.solve(y, tol=w.tol, max_iter=w.max_iter)
+    import torch
+    assert np.array_equal(h2, h_plain) and torch.equal(x2, x_plain)
+    s.close()
