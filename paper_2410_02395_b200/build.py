@@ -74,7 +74,7 @@ def build(force: bool = False, verbose: bool = False, sizes=None) -> str:
     if sizes:
         tag = "_".join(str(m) for m in sizes)
         jobs.append((os.path.join(CSRC, "fft_registry.cu"), os.path.join(OBJDIR, "fft_registry_dev_%s.o" % tag),
-                     ["-DMBS_DEV_SIZES=" + " ".join("X(%d)" % m for m in sizes)]))
+                     ["-DMBS_DEV_SIZES(X)=" + " ".join("X(%d)" % m for m in sizes)]))
     else:
         jobs.append((os.path.join(CSRC, "fft_registry.cu"), os.path.join(OBJDIR, "fft_registry.o"), []))
     for m in (sizes or fft_sizes()):

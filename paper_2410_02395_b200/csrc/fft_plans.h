@@ -51,7 +51,7 @@ template <> struct FftPlan<1260> { using type = GPlan<1260, 30, 30, 42>;      st
 
 // MBS_DEV_SIZES (build.py --sizes, kernel development only) restricts the library to a few sizes for quick rebuilds.
 #ifdef MBS_DEV_SIZES
-#define MBS_FOR_EACH_FFT_SIZE(X) MBS_DEV_SIZES
+#define MBS_FOR_EACH_FFT_SIZE(X) MBS_DEV_SIZES(X)
 #else
 #define MBS_FOR_EACH_FFT_SIZE(X) \
     X(8) X(16) X(32) X(64) X(128) X(256) X(512) X(1024) X(40) X(80) X(160) X(320) X(640) X(48) X(96) X(192) X(384) X(768) \
