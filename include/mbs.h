@@ -170,6 +170,22 @@ MBS_API int mbs_apply_operator(mbs_ctx* ctx, int which, const void* in_device, v
  * residual), MBS_ERR_INVALID_ARG (y identically zero: the relative residual of P:130 is undefined), or a
  * CUDA/state error.
  */
+/*
+ * out = B in (as mbs_apply_operator with MBS_OP_B; Eq. (8)) WITHOUT any allocation, for callers that may
+ * not call cudaMalloc (code under CUDA graph capture, serving loops, harnesses that forbid it).  The scratch of the
+ * edge-slab kernels (the compact correction buffers, sum over the axes with corrections of
+ * 16 t S_d (voxels / shape[d]) bytes, each rounded up to 256) lives in a static device array of
+ * MBS_STATIC_SCRATCH_BYTES that every GPU loading the library holds until the process exits.
+ *  - Grids that need more return MBS_ERR_INVALID_ARG (text in mbs_last_error); use mbs_apply_operator there.
+ *  - The array is shared by all contexts and calls on the device: calls that overlap on the GPU (different streams
+ *    with no ordering between them) race.  Calls on one stream are safe.  Asynchronous like mbs_apply_operator;
+ *    in == out allowed; device pointers, complex64, `shape`.
+ *  - Calls no cudaMalloc / cudaFree / allocating routine.  The first call on a device looks up the array's device
+ *    address (cudaGetSymbolAddress) with the context's device current.
+ */
+#define MBS_STATIC_SCRATCH_BYTES (16u << 20)
+MBS_API int mbs_apply_B_static(mbs_ctx* ctx, const void* in_device, void* out_device);
+
 MBS_API int mbs_solve(mbs_ctx* ctx, const void* y_device, void* x_device, double tol, int32_t max_iter,
               double* residual_history, int32_t* n_iter);
 

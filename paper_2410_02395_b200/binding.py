@@ -38,7 +38,8 @@ STATUS_NAMES = {0: "MBS_OK", 1: "MBS_ERR_INVALID_ARG", 2: "MBS_ERR_UNSUPPORTED_S
 DECLARED_SYMBOLS = ("mbs_create", "mbs_fft_supported", "mbs_workspace_bytes", "mbs_set_workspace", "mbs_set_option",
                     "mbs_set_potential", "mbs_apply_operator", "mbs_solve", "mbs_solve_host", "mbs_iterate",
                     "mbs_get_info", "mbs_get_kernel_stats", "mbs_reset_kernel_stats", "mbs_destroy", "mbs_last_error",
-                    "mbs_set_activation", "mbs_get_activation")
+                    "mbs_set_activation", "mbs_get_activation", "mbs_apply_B_static")
+MBS_STATIC_SCRATCH_BYTES = 16 << 20
 
 
 class mbs_info(ctypes.Structure):
@@ -75,6 +76,8 @@ _lib.mbs_set_potential.argtypes = [_vp, _vp]
 _lib.mbs_set_potential.restype = ctypes.c_int
 _lib.mbs_apply_operator.argtypes = [_vp, ctypes.c_int, _vp, _vp]
 _lib.mbs_apply_operator.restype = ctypes.c_int
+_lib.mbs_apply_B_static.argtypes = [_vp, _vp, _vp]
+_lib.mbs_apply_B_static.restype = ctypes.c_int
 _lib.mbs_solve.argtypes = [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int32, ctypes.POINTER(ctypes.c_double),
                            ctypes.POINTER(ctypes.c_int32)]
 _lib.mbs_solve.restype = ctypes.c_int
@@ -157,6 +160,11 @@ def mbs_set_potential(ctx, n_map_device_ptr: int):
 
 def mbs_apply_operator(ctx, which: int, in_ptr: int, out_ptr: int):
     _check(ctx, _lib.mbs_apply_operator(ctx, which, _vp(in_ptr), _vp(out_ptr)))
+
+
+def mbs_apply_B_static(ctx, in_ptr: int, out_ptr: int):
+    """out = B in with the slab scratch in the library's static device array: no allocation (include/mbs.h)."""
+    _check(ctx, _lib.mbs_apply_B_static(ctx, _vp(in_ptr), _vp(out_ptr)))
 
 
 def _solve(fn, ctx, y_ptr, x_ptr, tol, max_iter, want_history):

@@ -8,6 +8,7 @@
 
 #include <algorithm>
 #include <complex>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1238,5 +1239,72 @@ extern "C" int mbs_get_info(const mbs_ctx* c, mbs_info* out) {
     out->workspace_bytes = c->ws_bytes;
     out->kernel_launches = c->launches;
     out->last_solve_ms = c->last_solve_ms;
+    return MBS_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// mbs_apply_B_static: the scattering operator B = I - V (Eq. (8)) for callers that may not allocate
+// (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  The edge-slab kernels need scratch:
+// the compact correction buffers corr_d(in) that the pointwise pass then subtracts.  mbs_apply_operator keeps them in
+// the context's workspace; this variant keeps them in a file-scope device array of MBS_STATIC_SCRATCH_BYTES, which
+// every GPU that loads the library holds until the process exits.  Same kernels, same launch geometry, same results.
+//  - no cudaMalloc / cudaFree / allocating library call on this path (and no event creation: launches are not profiled);
+//  - the array is shared by every call and every context on the device and keeps the last call's contents: the slab
+//    kernels overwrite every slot they later read, and the range in use is cleared first all the same; two calls that
+//    overlap on the GPU (different streams, no ordering between them) race on it;
+//  - in host code `g_static_scratch` is only the host-side stand-in of the symbol: its device address is looked up once
+//    per device with cudaGetSymbolAddress, with that device current, and that pointer is what the kernels get.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned char g_static_scratch[MBS_STATIC_SCRATCH_BYTES];
+
+static int static_scratch_address(mbs_ctx* c, unsigned char** out) {
+    constexpr int MAX_DEV = 64;
+    static unsigned char* addr[MAX_DEV] = {nullptr};
+    static std::mutex mu;
+    int dev = 0;
+    MBS_CUDA(c, cudaGetDevice(&dev));
+    if (dev < 0 || dev >= MAX_DEV) return fail(c, MBS_ERR_INVALID_ARG, "device ordinal %d out of range", dev);
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        MBS_CUDA(c, cudaGetSymbolAddress(&p, g_static_scratch));
+        if (!p || ((uintptr_t)p & 255) != 0) return fail(c, MBS_ERR_CUDA, "cudaGetSymbolAddress returned an unusable address");
+        addr[dev] = (unsigned char*)p;
+    }
+    *out = addr[dev];
+    return MBS_OK;
+}
+
+extern "C" int mbs_apply_B_static(mbs_ctx* c, const void* in_device, void* out_device) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (!c->potential_set) return fail(c, MBS_ERR_STATE, "mbs_set_potential has not been called");
+    if (!in_device || !out_device) return fail(c, MBS_ERR_INVALID_ARG, "NULL array argument");
+    const GridDesc& g = c->g;
+    size_t off[3] = {0, 0, 0}, need = 0;
+    for (int ax = 0; ax < 3; ++ax) {
+        off[ax] = need;
+        need += align_up(sizeof(cf) * corr_elems(g, ax));
+    }
+    if (need > (size_t)MBS_STATIC_SCRATCH_BYTES)
+        return fail(c, MBS_ERR_INVALID_ARG,
+                    "mbs_apply_B_static: the edge corrections of this grid need %zu bytes of scratch, the static array holds %zu "
+                    "(MBS_STATIC_SCRATCH_BYTES); use mbs_apply_operator", need, (size_t)MBS_STATIC_SCRATCH_BYTES);
+    unsigned char* base = nullptr;
+    MBS_TRY(static_scratch_address(c, &base));
+    if (need) MBS_CUDA(c, cudaMemsetAsync(base, 0, need, c->stream));
+    CorrBufs cb{};
+    for (int ax = 0; ax < 3; ++ax) cb.buf[ax] = corr_elems(g, ax) ? reinterpret_cast<cf*>(base + off[ax]) : nullptr;
+    for (int ax = 0; ax < 3; ++ax) {
+        if (!cb.buf[ax]) continue;
+        SlabParams sp{};
+        sp.in = (const cf*)in_device; sp.in2 = nullptr; sp.out = cb.buf[ax]; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
+        sp.compact_in = 0; sp.state = c->state; sp.check_done = 0;
+        c->launches++;
+        MBS_CUDA(c, launch_slab(g, sp, c->stream));
+    }
+    PointwiseParams p = pw_defaults(c, false);
+    p.in = (const cf*)in_device; p.bdiag = c->bdiag; p.out = (cf*)out_device; p.corr = cb; p.reduce = RED_NONE;
+    c->launches++;
+    MBS_CUDA(c, launch_pointwise(g, p, c->num_sms, c->stream));
     return MBS_OK;
 }
