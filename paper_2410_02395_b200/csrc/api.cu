@@ -86,6 +86,7 @@ struct mbs_ctx {
     int use_graph = -1;      // -1 = automatic
     int use_tma = 1;         // TMA-fed strided sweeps
     int use_line = 1;        // warp-line first / last sweeps
+    int slab_one_launch = 0; // slab passes of all axes in one launch (k_slab_pass_all) instead of one launch per axis
     int use_merge = 0;       // last sweep merged with the next iteration's first sweep (measured slower: off by default)
     bool u_ready = false;    // u already holds the next iteration's first sweep on the rows outside the axis-0/1 slabs
 
@@ -475,8 +476,9 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
         case MBS_OPT_USE_GRAPH: c->use_graph = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_PROFILE: c->profile = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_TMA: c->use_tma = value ? 1 : 0; return MBS_OK;
-        case MBS_OPT_LINE: c->use_line = value ? 1 : 0; return MBS_OK;
+        case MBS_OPT_LINE: c->use_line = value == 2 ? 2 : (value ? 1 : 0); return MBS_OK;
         case MBS_OPT_MERGE: c->use_merge = value ? 1 : 0; return MBS_OK;
+        case MBS_OPT_SLAB_FUSED: c->slab_one_launch = value ? 1 : 0; invalidate_graph(c); return MBS_OK;
         case MBS_OPT_REFINE: c->refine = value < 0 ? -1 : (value ? 1 : 0); invalidate_graph(c); return MBS_OK;
         default: return fail(c, MBS_ERR_INVALID_ARG, "unknown option %d", option);
     }
@@ -741,6 +743,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     p.n_tiles = (p.n_lines + e->CC - 1) / e->CC;
     p.partials = c->partials; p.state = c->state; p.hist = c->hist_dev; p.reduce_mode = RED_RESIDUAL;
     p.dref = c->split ? c->dref : nullptr;
+    p.line_variant = c->use_line == 2 ? 1 : 0;
     const double vb = 8.0 * (double)g.voxels;
     if (c->ndim == 1) {
         p.slot0 = 0; p.finish = 1;
@@ -802,7 +805,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
             c->u_ready = true;
             return MBS_OK;
         }
-        const int nb5 = e->line_blocks(LINE_S5, g.t, p.n_lines, c->num_sms);
+        const int nb5 = e->line_blocks(LINE_S5, g.t, p.line_variant, p.n_lines, c->num_sms);
         if (nb5 < 1) return fail(c, MBS_ERR_CUDA, "line sweep: occupancy query failed");
         const int mask = mask01 | (e2 ? 4 : 0);
         p.slot0 = 0; p.n_total = nb5; p.finish = mask ? 0 : 1;
@@ -810,7 +813,18 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
             KernelScope ks(c, "line_sweep5", 4 * vb);
             MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S5, done, c->num_sms, c->stream));
         }
-        if (mask && slab_pass_supported(g.t)) {
+        if (mask && slab_pass_supported(g.t) && c->slab_one_launch) {
+            // corr_d(d) of every axis from the compact d and the finish of the slab voxels, one launch (k_slab_pass_all)
+            SlabPassParams sp{};
+            sp.u = c->u; sp.x = x; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.alpha = (float)c->alpha;
+            sp.partials = c->partials; sp.slot0 = nb5; sp.state = c->state; sp.hist = c->hist_dev;
+            sp.active = act_on ? c->act.flags : nullptr;
+            const cf* dsv[3] = {c->ds.buf[0], c->ds.buf[1], c->ds.buf[2]};
+            const double vox = (double)((mask & 1) ? corr_elems(g, 0) : 0) + (double)((mask & 2) ? corr_elems(g, 1) : 0) +
+                               (double)((mask & 4) ? corr_elems(g, 2) : 0);
+            KernelScope ks(c, "slab_pass_all", 40.0 * vox);
+            MBS_CUDA(c, launch_slab_pass_all(g, sp, dsv, mask, c->stream));
+        } else if (mask && slab_pass_supported(g.t)) {
             // one pass per axis: corr_ax(d) from the compact d, applied in the same kernel; the last pass finishes
             int slot = nb5, last_ax = (mask & 4) ? 2 : ((mask & 2) ? 1 : 0);
             for (int ax = 0; ax < 3; ++ax) {

@@ -5,6 +5,7 @@
 #include "fused_kernels.cuh"
 #include "fft_tma.cuh"
 #include "line_kernels.cuh"
+#include "line_fast.cuh"
 #include "line_merged.cuh"
 
 #ifndef MBS_FFT_SIZE
@@ -103,13 +104,28 @@ constexpr int LINE_WARPS = 8;
 #ifndef MBS_LINE_MINB_S1
 #define MBS_LINE_MINB_S1 3
 #endif
-template <int MODE>
+// FAST: the variant with t = 8 known at compile time (line_fast.cuh), chosen on the host when the context has t = 8.
+// Measured A/B on one box (profiles/r02_line_kernels.md): with two or more lines per warp (T <= 16, e.g. the 256-long lines
+// of config 3) the first sweep gains 12 %; with one 512-long line per warp it loses 10 % (it no longer fits the 80 registers
+// that three CTAs per SM allow), while the last sweep gains 3 % there and loses 3 % at T = 16.  So: first sweep for T <= 16,
+// last sweep for T = 32.
+template <int MODE> constexpr bool line_fast_avail() {
+    if constexpr (line_ok())
+        return line_fast_ok<PL, 8>() && !line_stage_b<PL, MODE>() && (MODE == LINE_S1 ? PL::T <= 16 : PL::T == 32);
+    else
+        return false;
+}
+template <int MODE, bool ACT = false, bool FAST = false>
 __global__ void __launch_bounds__(LINE_WARPS * 32, MODE == LINE_S1 ? MBS_LINE_MINB_S1 : 2) k_line(const FusedParams p, const cf* __restrict__ tw,
                                                                          const int* __restrict__ done) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ double red[32];
     if (done && *done) return;
-    if constexpr (line_ok()) line_body<PL, LINE_WARPS, MODE>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
+    if constexpr (FAST) {
+        if constexpr (line_fast_avail<MODE>()) line_body_fast<PL, LINE_WARPS, MODE, ACT, 8>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
+    } else {
+        if constexpr (line_ok()) line_body<PL, LINE_WARPS, MODE, ACT>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
+    }
 }
 
 // last sweep merged with the next iteration's first sweep (line_merged.cuh); G = warps per grid row
@@ -242,14 +258,24 @@ int fused_blocks_entry(int mode, int t, long long n_tiles, int num_sms) {
     return e == cudaSuccess ? nb : -1;
 }
 
+typedef void (*LineKernel)(const FusedParams, const cf*, const int*);
 template <int MODE>
-cudaError_t line_grid(int t, long long n_lines, int num_sms, int* nb_out, size_t* smem_out) {
+LineKernel line_kernel(bool act, bool fast) {
+    if (fast) return act ? k_line<MODE, true, true> : k_line<MODE, false, true>;
+    return act ? k_line<MODE, true, false> : k_line<MODE, false, false>;
+}
+
+// grid of the plain (not ACT) kernel of the variant the context's t selects; the ACT kernels are launched on the same grid
+// (the number of residual partials is fixed by line_blocks())
+template <int MODE>
+cudaError_t line_grid(int t, int variant, long long n_lines, int num_sms, int* nb_out, size_t* smem_out, bool* fast_out) {
     if constexpr (!line_ok()) {
         return cudaErrorNotSupported;
     } else {
+        const bool fast = line_fast_avail<MODE>() && t == 8 && variant == 0;
         const size_t smem = line_smem_bytes<PL, LINE_WARPS, MODE>(t);
         int bps = 1;
-        cudaError_t e = prepare(k_line<MODE>, LINE_WARPS * 32, smem, &bps);
+        cudaError_t e = prepare(line_kernel<MODE>(false, fast), LINE_WARPS * 32, smem, &bps);
         if (e != cudaSuccess) return e;
         const long long units = (n_lines + (32 / PL::T) - 1) / (32 / PL::T);
         long long nb = (long long)num_sms * bps;
@@ -259,23 +285,26 @@ cudaError_t line_grid(int t, long long n_lines, int num_sms, int* nb_out, size_t
         if (nb < 1) nb = 1;
         *nb_out = (int)nb;
         *smem_out = smem;
+        *fast_out = fast;
         return cudaSuccess;
     }
 }
 
-cudaError_t line_entry(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st) {
-    int nb = 1;
+template <int MODE>
+cudaError_t line_launch(const FusedParams& p, const cf* tw, const int* done, int num_sms, cudaStream_t st) {
+    int nb = 1, bps = 1;
     size_t smem = 0;
-    if (mode == LINE_S1) {
-        cudaError_t e = line_grid<LINE_S1>(p.t, p.n_lines, num_sms, &nb, &smem);
-        if (e != cudaSuccess) return e;
-        k_line<LINE_S1><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
-    } else {
-        cudaError_t e = line_grid<LINE_S5>(p.t, p.n_lines, num_sms, &nb, &smem);
-        if (e != cudaSuccess) return e;
-        k_line<LINE_S5><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
-    }
+    bool fast = false;
+    cudaError_t e = line_grid<MODE>(p.t, p.line_variant, p.n_lines, num_sms, &nb, &smem, &fast);
+    if (e != cudaSuccess) return e;
+    const LineKernel k = line_kernel<MODE>(p.active != nullptr, fast);
+    if (p.active && (e = prepare(k, LINE_WARPS * 32, smem, &bps)) != cudaSuccess) return e;
+    k<<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
     return cudaGetLastError();
+}
+
+cudaError_t line_entry(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st) {
+    return mode == LINE_S1 ? line_launch<LINE_S1>(p, tw, done, num_sms, st) : line_launch<LINE_S5>(p, tw, done, num_sms, st);
 }
 
 // warps per grid row for the merged sweep, 0 if the row does not map onto whole warps of one CTA
@@ -355,11 +384,12 @@ int merged_blocks_entry(int S2, int t, long long n_lines, int num_sms) {
     return e == cudaSuccess ? nb : 0;
 }
 
-int line_blocks_entry(int mode, int t, long long n_lines, int num_sms) {
+int line_blocks_entry(int mode, int t, int variant, long long n_lines, int num_sms) {
     int nb = 1;
     size_t smem = 0;
-    cudaError_t e = (mode == LINE_S1) ? line_grid<LINE_S1>(t, n_lines, num_sms, &nb, &smem)
-                                      : line_grid<LINE_S5>(t, n_lines, num_sms, &nb, &smem);
+    bool fast = false;
+    cudaError_t e = (mode == LINE_S1) ? line_grid<LINE_S1>(t, variant, n_lines, num_sms, &nb, &smem, &fast)
+                                      : line_grid<LINE_S5>(t, variant, n_lines, num_sms, &nb, &smem, &fast);
     return e == cudaSuccess ? nb : -1;
 }
 

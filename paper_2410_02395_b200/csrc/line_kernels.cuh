@@ -133,7 +133,9 @@ __device__ __forceinline__ unsigned line_slab_row(const FusedParams& p, unsigned
     return (unsigned)i0 * (unsigned)p.N1 + (unsigned)i1;
 }
 
-template <class PL, int NWARP, int MODE>
+// ACT: subdomain activation -- lines of inactive subdomains are skipped; a separate instantiation so that
+// the plain kernels keep their code exactly
+template <class PL, int NWARP, int MODE, bool ACT = false>
 __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __restrict__ tw_global, cf* smem, double* red) {
     constexpr int M = PL::M, P = PL::P, T = PL::T, NT = NWARP * 32;
     static_assert(T <= 32 && 32 % T == 0, "a line must fit in one warp");
@@ -156,19 +158,21 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
     float acc = 0.f;
     for (unsigned unit = blockIdx.x * NWARP + warp; unit < n_units; unit += gridDim.x * NWARP) {
         unsigned line = unit * LW + lsub;
-        bool valid = line < n_lines;
+        const bool in_range = line < n_lines;
         unsigned row = line / (unsigned)p.S2;
         const int seg = (int)(line - row * (unsigned)p.S2);
         if (MODE == LINE_S1 && p.slab_rows_only) {    // `line` counted slab-row lines: map to the real row
-            row = valid ? line_slab_row(p, row) : 0u;
+            row = in_range ? line_slab_row(p, row) : 0u;
             line = row * (unsigned)p.S2 + (unsigned)seg;
         }
         const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
-        if (p.active) {
-            // subdomain activation: the lines of an inactive subdomain are not computed
-            if (valid) valid = p.active[((i0 / p.M0) * p.S1 + i1 / p.M1) * p.S2 + seg] != 0;
-            if (!__any_sync(0xffffffffu, valid)) continue;
+        bool act_ok = true;
+        if constexpr (ACT) {
+            // the lines of an inactive subdomain are not computed
+            act_ok = in_range && p.active[((i0 / p.M0) * p.S1 + i1 / p.M1) * p.S2 + seg] != 0;
+            if (!__any_sync(0xffffffffu, act_ok)) continue;
         }
+        const bool valid = in_range && act_ok;
         long long o0 = -1, o1 = -1;                   // compact row offsets of the axis-0 / axis-1 slabs
         if (valid && p.e0) {
             const int q = line_edge_slot(i0, p.M0, t);
@@ -219,10 +223,12 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
             if (!p.slab_rows_only) {
                 const unsigned nline = (unit + gridDim.x * NWARP) * LW + lsub;
                 bool want = nline < n_lines;
-                if (want && p.active) {
-                    const unsigned nrow = nline / (unsigned)p.S2;
-                    const int ni0 = (int)(nrow / (unsigned)p.N1), ni1 = (int)(nrow - (unsigned)ni0 * (unsigned)p.N1);
-                    want = p.active[((ni0 / p.M0) * p.S1 + ni1 / p.M1) * p.S2 + (int)(nline - nrow * (unsigned)p.S2)] != 0;
+                if constexpr (ACT) {
+                    if (want) {
+                        const unsigned nrow = nline / (unsigned)p.S2;
+                        const int ni0 = (int)(nrow / (unsigned)p.N1), ni1 = (int)(nrow - (unsigned)ni0 * (unsigned)p.N1);
+                        want = p.active[((ni0 / p.M0) * p.S1 + ni1 / p.M1) * p.S2 + (int)(nline - nrow * (unsigned)p.S2)] != 0;
+                    }
                 }
                 if (want) {
                     const char* nx = reinterpret_cast<const char*>(p.x + (long long)nline * M);

@@ -127,6 +127,10 @@ struct SlabPassParams {
 int slab_pass_blocks(const GridDesc& g, int ax);
 bool slab_pass_supported(int t);
 cudaError_t launch_slab_pass(const GridDesc& g, const SlabPassParams& p, cudaStream_t st);
+// all axes of `mask` in one launch (k_slab_pass_all): p.ds / p.axis / p.e1 / p.e2 / p.finish of `p` are not used; the
+// launch writes slab_pass_all_blocks(g, mask) partials from p.slot0 on and finishes the iteration
+int slab_pass_all_blocks(const GridDesc& g, int mask);
+cudaError_t launch_slab_pass_all(const GridDesc& g, const SlabPassParams& p, const cf* const ds[3], int mask, cudaStream_t st);
 int fixup_blocks(const GridDesc& g, int e0, int e1, int e2, int num_sms);
 cudaError_t launch_fixup(const GridDesc& g, const FixupParams& p, int nblocks, cudaStream_t st);
 cudaError_t launch_row_mask(const cf* y, unsigned char* mask, long long rows, int N2, cudaStream_t st);
@@ -182,6 +186,7 @@ struct FusedParams {
     double* hist;
     const int* active;   // subdomain activation: flags per subdomain, or nullptr; lines of an inactive
                          // subdomain are skipped by the warp-line sweeps
+    int line_variant;    // warp-line sweeps: 0 = the variant with t known at compile time when there is one (t = 8), 1 = generic
     const cf* dref;      // split iterate (api.cu "refinement"): the sweeps run on the small part delta of x = x_ref + delta,
                          // and the last sweep adds d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec) to d = delta - u'; or nullptr
 };
@@ -223,7 +228,7 @@ struct FftEntry {
     int (*fused_blocks)(int mode, int t, long long n_tiles, int num_sms);
     // warp-line variant of the first / last sweep (line_kernels.cuh); nullptr when a line does not fit in a warp
     cudaError_t (*line)(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st);
-    int (*line_blocks)(int mode, int t, long long n_lines, int num_sms);
+    int (*line_blocks)(int mode, int t, int variant, long long n_lines, int num_sms);   // variant: FusedParams::line_variant
     // last sweep merged with the next iteration's first sweep (line_merged.cuh); merged_blocks = grid size, 0 if the
     // number of subdomains along the last axis does not map onto whole warps of one CTA
     cudaError_t (*merged)(const FusedParams& p, const cf* tw, const int* done, int num_sms, cudaStream_t st);
