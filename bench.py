@@ -71,7 +71,7 @@ def parse_args():
     ap.add_argument("--no-other-configs", action="store_true", help="default run: do not time configs 3 and 4 as well")
     ap.add_argument("--unfused", action="store_true", help="one kernel per step of P:122-128 instead of the fused sweeps")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
-                    help="kernel option for profiling runs, e.g. MERGE=1, LINE=0, TMA=0 (enum mbs_option; not the headline)")
+                    help="kernel option for profiling runs, e.g. LINE=2, LINE=0, TMA=0 (enum mbs_option; not the headline)")
     ap.add_argument("--activation", type=float, default=None, metavar="THRESHOLD",
                     help="--converge-config only: solve with subdomain activation (P:139-141) at this relative threshold "
                          "(negative: the default tol / 10) and report it beside the plain solve")

@@ -74,15 +74,10 @@ enum mbs_option {
                                    the contiguous axis, no block barriers), in the variant with t = 8 known at compile
                                    time where it is the faster one; 2: warp-line kernels, generic-t variant only;
                                    0: tile kernels with in-CTA edge terms                                          */
-    MBS_OPT_MERGE = 6,          /* 1: the last sweep also runs the next iteration's first sweep on every row outside the
-                                   axis-0/1 slabs (saves the re-read of x and B_diag, 96 B ledger); needs MBS_OPT_LINE.
-                                   Default 0: with 128 registers per thread it is latency-bound and measured slower  */
     MBS_OPT_REFINE = 7,         /* split iterate x = x_ref + delta (api.cu recenter()): the FFT sweeps run on the small part
                                    delta, so the complex64 rounding floor of the residual falls with it and tolerances such
                                    as config 1's 1e-6 are reachable; same iteration in exact arithmetic, two extra arrays.
                                    -1 (default): on for grids of <= 2^21 voxels; 0: off; 1: on                   */
-    MBS_OPT_SLAB_FUSED = 8,     /* 1: the slab passes of all axes (corr_d(d), residual and update at the slab voxels) run as
-                                   one launch in which every slab voxel has one owner; 0 (default): one launch per axis */
     MBS_OPT_PROFILE = 3         /* 1: bracket every kernel launch with CUDA events on the context's stream and
                                    accumulate per-kernel device time (mbs_get_kernel_stats); disables graphs   */
 };

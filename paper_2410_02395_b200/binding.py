@@ -28,9 +28,7 @@ MBS_OK, MBS_ERR_INVALID_ARG, MBS_ERR_UNSUPPORTED_SIZE, MBS_ERR_OOM = 0, 1, 2, 3
 MBS_ERR_CUDA, MBS_ERR_NOT_CONVERGED, MBS_ERR_NUMERIC, MBS_ERR_STATE = 4, 5, 6, 7
 MBS_OP_B, MBS_OP_PROPAGATOR, MBS_OP_A, MBS_OP_PRECOND_A = 0, 1, 2, 3
 MBS_OPT_FUSED, MBS_OPT_CHECK_INTERVAL, MBS_OPT_USE_GRAPH, MBS_OPT_PROFILE, MBS_OPT_TMA, MBS_OPT_LINE = 0, 1, 2, 3, 4, 5
-MBS_OPT_MERGE = 6
 MBS_OPT_REFINE = 7
-MBS_OPT_SLAB_FUSED = 8
 
 STATUS_NAMES = {0: "MBS_OK", 1: "MBS_ERR_INVALID_ARG", 2: "MBS_ERR_UNSUPPORTED_SIZE", 3: "MBS_ERR_OOM",
                 4: "MBS_ERR_CUDA", 5: "MBS_ERR_NOT_CONVERGED", 6: "MBS_ERR_NUMERIC", 7: "MBS_ERR_STATE"}

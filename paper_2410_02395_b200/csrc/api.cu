@@ -86,9 +86,6 @@ struct mbs_ctx {
     int use_graph = -1;      // -1 = automatic
     int use_tma = 1;         // TMA-fed strided sweeps
     int use_line = 1;        // warp-line first / last sweeps
-    int slab_one_launch = 0; // slab passes of all axes in one launch (k_slab_pass_all) instead of one launch per axis
-    int use_merge = 0;       // last sweep merged with the next iteration's first sweep (measured slower: off by default)
-    bool u_ready = false;    // u already holds the next iteration's first sweep on the rows outside the axis-0/1 slabs
 
     int profile = 0;
     Profiler prof;
@@ -477,8 +474,6 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
         case MBS_OPT_PROFILE: c->profile = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_TMA: c->use_tma = value ? 1 : 0; return MBS_OK;
         case MBS_OPT_LINE: c->use_line = value == 2 ? 2 : (value ? 1 : 0); return MBS_OK;
-        case MBS_OPT_MERGE: c->use_merge = value ? 1 : 0; return MBS_OK;
-        case MBS_OPT_SLAB_FUSED: c->slab_one_launch = value ? 1 : 0; invalidate_graph(c); return MBS_OK;
         case MBS_OPT_REFINE: c->refine = value < 0 ? -1 : (value ? 1 : 0); invalidate_graph(c); return MBS_OK;
         default: return fail(c, MBS_ERR_INVALID_ARG, "unknown option %d", option);
     }
@@ -490,7 +485,7 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
 static bool fused_available(const mbs_ctx* c);
 static bool activation_effective(const mbs_ctx* c) {
     return c->activation && c->ndim >= 2 && c->fused && fused_available(c) && c->use_line && c->fft[2]->line &&
-           !c->use_merge && slab_pass_supported(c->g.t);
+           slab_pass_supported(c->g.t);
 }
 
 extern "C" int mbs_set_activation(mbs_ctx* c, int enable, double threshold) {
@@ -733,7 +728,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     const int* done = &c->state->done;
     FusedParams p{};
     p.x = x; p.bdiag = c->bdiag; p.y = y; p.ymask = c->ymask; p.ysc = to_cf(-c->c); p.u = c->u;
-    p.N0 = g.N[0]; p.S0 = g.S[0]; p.slab_rows_only = 0;
+    p.N0 = g.N[0]; p.S0 = g.S[0];
     p.N1 = g.N[1]; p.N2 = g.N[2]; p.S2 = g.S[2]; p.a2 = g.a[2]; p.per2 = g.per[2]; p.t = g.t;
     p.e0 = e0; p.e1 = e1; p.M0 = g.M[0]; p.M1 = g.M[1]; p.S1 = g.S[1];
     p.cx0 = c->cx.buf[0]; p.cx1 = c->cx.buf[1]; p.ds0 = c->ds.buf[0]; p.ds1 = c->ds.buf[1];
@@ -765,46 +760,11 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
         // warp-line sweeps: corr_2(x) inside sweep 1; corr_2(d) through the compact buffers like axes 0 and 1
         const int e2 = g.a[2] > 0 ? 1 : 0;
         p.ds2 = c->ds.buf[2];
-        const int nb51 = (c->use_merge && e->merged && slab_pass_supported(g.t))
-                             ? e->merged_blocks(g.S[2], g.t, p.n_lines, c->num_sms) : 0;
-        const bool merge = nb51 > 0;
-        if (!(merge && c->u_ready)) {
+        {
             KernelScope ks(c, "line_sweep1", (3.0 + c->y_row_fraction) * vb);     // all-zero rows of y are not read
             MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S1, done, c->num_sms, c->stream));
-        } else if (mask01) {
-            // u of the rows outside the slabs was written by the merged sweep of the iteration before; the slab rows
-            // follow now that the slab passes have finished their x
-            const long long nE0 = e0 ? (long long)g.S[0] * 2 * g.t : 0, nE1 = e1 ? (long long)g.S[1] * 2 * g.t : 0;
-            const long long slab_rows = nE0 * g.N[1] + (g.N[0] - nE0) * nE1;
-            FusedParams ps = p;
-            ps.slab_rows_only = 1;
-            ps.n_lines = slab_rows * g.S[2];
-            KernelScope ks(c, "line_sweep1_slab_rows", 32.0 * (double)slab_rows * g.N[2]);
-            MBS_CUDA(c, e->line(ps, c->tw_dev[2], LINE_S1, done, c->num_sms, c->stream));
         }
         MBS_TRY(run_middle_sweeps(c, c->u, 1, true));
-        if (merge) {
-            p.slot0 = 0; p.n_total = nb51; p.finish = mask01 ? 0 : 1;
-            {
-                KernelScope ks(c, "line_sweep51", 5 * vb);                            // reads u, x, B_diag; writes x, u
-                MBS_CUDA(c, e->merged(p, c->tw_dev[2], done, c->num_sms, c->stream));
-            }
-            int slot = nb51;
-            const int last_ax = (mask01 & 2) ? 1 : 0;
-            for (int ax = 0; ax < 2; ++ax) {
-                if (!((mask01 >> ax) & 1)) continue;
-                SlabPassParams sp{};
-                sp.ds = c->ds.buf[ax]; sp.u = c->u; sp.x = x; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
-                sp.e1 = e1; sp.e2 = 0; sp.alpha = (float)c->alpha; sp.partials = c->partials; sp.slot0 = slot;
-                sp.finish = (ax == last_ax) ? 1 : 0; sp.state = c->state; sp.hist = c->hist_dev;
-                static const char* names[2] = {"slab_pass_ax0", "slab_pass_ax1"};
-                KernelScope ks(c, names[ax], 40.0 * (double)corr_elems(g, ax));
-                MBS_CUDA(c, launch_slab_pass(g, sp, c->stream));
-                slot += slab_pass_blocks(g, ax);
-            }
-            c->u_ready = true;
-            return MBS_OK;
-        }
         const int nb5 = e->line_blocks(LINE_S5, g.t, p.line_variant, p.n_lines, c->num_sms);
         if (nb5 < 1) return fail(c, MBS_ERR_CUDA, "line sweep: occupancy query failed");
         const int mask = mask01 | (e2 ? 4 : 0);
@@ -813,18 +773,7 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
             KernelScope ks(c, "line_sweep5", 4 * vb);
             MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S5, done, c->num_sms, c->stream));
         }
-        if (mask && slab_pass_supported(g.t) && c->slab_one_launch) {
-            // corr_d(d) of every axis from the compact d and the finish of the slab voxels, one launch (k_slab_pass_all)
-            SlabPassParams sp{};
-            sp.u = c->u; sp.x = x; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.alpha = (float)c->alpha;
-            sp.partials = c->partials; sp.slot0 = nb5; sp.state = c->state; sp.hist = c->hist_dev;
-            sp.active = act_on ? c->act.flags : nullptr;
-            const cf* dsv[3] = {c->ds.buf[0], c->ds.buf[1], c->ds.buf[2]};
-            const double vox = (double)((mask & 1) ? corr_elems(g, 0) : 0) + (double)((mask & 2) ? corr_elems(g, 1) : 0) +
-                               (double)((mask & 4) ? corr_elems(g, 2) : 0);
-            KernelScope ks(c, "slab_pass_all", 40.0 * vox);
-            MBS_CUDA(c, launch_slab_pass_all(g, sp, dsv, mask, c->stream));
-        } else if (mask && slab_pass_supported(g.t)) {
+        if (mask && slab_pass_supported(g.t)) {
             // one pass per axis: corr_ax(d) from the compact d, applied in the same kernel; the last pass finishes
             int slot = nb5, last_ax = (mask & 4) ? 2 : ((mask & 2) ? 1 : 0);
             for (int ax = 0; ax < 3; ++ax) {
@@ -930,7 +879,7 @@ extern "C" int mbs_apply_operator(mbs_ctx* c, int which, const void* in_device, 
 // ---------------------------------------------------------------------------------------------
 static bool split_effective(const mbs_ctx* c) {
     const bool want = c->refine == 1 || (c->refine < 0 && c->g.voxels <= (1LL << 21));
-    return want && c->fused && fused_available(c) && !c->use_merge && !c->activation;
+    return want && c->fused && fused_available(c) && !c->activation;
 }
 
 static int recenter(mbs_ctx* c, const cf* y, cf* x, bool add_delta) {
@@ -964,9 +913,8 @@ static int recenter(mbs_ctx* c, const cf* y, cf* x, bool add_delta) {
 
 // Reset the device state for a new solve and (nu <= 0) compute nu = || B (L+I)^-1 y_vec ||
 static int begin_solve(mbs_ctx* c, const cf* y, const cf* x, double tol, int32_t max_iter, double nu) {
-    c->u_ready = false;                               // the workspace u is scratch between solves
     if (c->activation && !activation_effective(c))
-        return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation needs the default kernel options (fused warp-line sweeps, no merge)");
+        return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation needs the default kernel options (fused warp-line sweeps)");
     DevState init{};
     init.iter = 0; init.done = 0; init.max_iter = max_iter; init.ticket = 0; init.tol = tol;
     init.nu2 = nu > 0 ? nu * nu : 0.0; init.last_sum = 0;
@@ -1056,7 +1004,7 @@ static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_g
         return MBS_OK;
     }
     const bool stale = !c->graph_exec || c->graph_y != y || c->graph_x != x || c->graph_batch != batch || c->graph_split != (int)c->split ||
-                       c->graph_fused != c->fused || c->graph_tma != c->use_tma || c->graph_line != c->use_line * 2 + c->use_merge;
+                       c->graph_fused != c->fused || c->graph_tma != c->use_tma || c->graph_line != c->use_line;
     if (stale) {
         if (c->graph_exec) { cudaGraphExecDestroy(c->graph_exec); c->graph_exec = nullptr; }
         if (!c->cap_stream) MBS_CUDA(c, cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking));
@@ -1077,7 +1025,7 @@ static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_g
         cudaGraphDestroy(graph);
         if (e2 != cudaSuccess) { c->graph_exec = nullptr; return fail(c, MBS_ERR_CUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e2)); }
         c->graph_y = y; c->graph_x = x; c->graph_batch = batch; c->graph_split = (int)c->split;
-        c->graph_fused = c->fused; c->graph_tma = c->use_tma; c->graph_line = c->use_line * 2 + c->use_merge;
+        c->graph_fused = c->fused; c->graph_tma = c->use_tma; c->graph_line = c->use_line;
         c->launches_per_batch = captured;
     }
     MBS_CUDA(c, cudaGraphLaunch(c->graph_exec, c->stream));

@@ -6,7 +6,6 @@
 #include "fft_tma.cuh"
 #include "line_kernels.cuh"
 #include "line_fast.cuh"
-#include "line_merged.cuh"
 
 #ifndef MBS_FFT_SIZE
 #error "compile with -DMBS_FFT_SIZE=<M>"
@@ -126,16 +125,6 @@ __global__ void __launch_bounds__(LINE_WARPS * 32, MODE == LINE_S1 ? MBS_LINE_MI
     } else {
         if constexpr (line_ok()) line_body<PL, LINE_WARPS, MODE, ACT>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
     }
-}
-
-// last sweep merged with the next iteration's first sweep (line_merged.cuh); G = warps per grid row
-template <int G>
-__global__ void __launch_bounds__(LINE_WARPS * 32, 2) k_line_merged(const FusedParams p, const cf* __restrict__ tw,
-                                                                    const int* __restrict__ done) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ double red[32];
-    if (done && *done) return;
-    if constexpr (line_ok()) line_merged_body<PL, LINE_WARPS, G>(p, tw, reinterpret_cast<cf*>(smem_raw), red);
 }
 
 // Opt in to the dynamic shared memory a kernel needs and query its occupancy; cached per (kernel, size).
@@ -307,83 +296,6 @@ cudaError_t line_entry(const FusedParams& p, const cf* tw, int mode, const int* 
     return mode == LINE_S1 ? line_launch<LINE_S1>(p, tw, done, num_sms, st) : line_launch<LINE_S5>(p, tw, done, num_sms, st);
 }
 
-// warps per grid row for the merged sweep, 0 if the row does not map onto whole warps of one CTA
-int merged_group(int S2) {
-    if constexpr (!line_ok()) {
-        return 0;
-    } else {
-        constexpr int LW = 32 / PL::T;
-        if (LW % S2 == 0) return 1;
-        if (S2 % LW == 0) {
-            const int g = S2 / LW;
-            if (g == 2 || g == 4 || g == 8) return g;
-        }
-        return 0;
-    }
-}
-
-template <int G>
-cudaError_t merged_grid(int t, long long n_lines, int num_sms, int* nb_out, size_t* smem_out) {
-    if constexpr (!line_ok()) {
-        return cudaErrorNotSupported;
-    } else {
-        const size_t smem = line_merged_smem_bytes<PL, LINE_WARPS>(t);
-        int bps = 1;
-        cudaError_t e = prepare(k_line_merged<G>, LINE_WARPS * 32, smem, &bps);
-        if (e != cudaSuccess) return e;
-        const long long units = (n_lines + (32 / PL::T) - 1) / (32 / PL::T);
-        long long nb = (long long)num_sms * bps;
-        const long long need = (units + LINE_WARPS - 1) / LINE_WARPS;
-        if (nb > need) nb = need;
-        if (nb > MBS_MAX_PARTIALS / 2) nb = MBS_MAX_PARTIALS / 2;
-        if (nb < 1) nb = 1;
-        *nb_out = (int)nb;
-        *smem_out = smem;
-        return cudaSuccess;
-    }
-}
-
-cudaError_t merged_entry(const FusedParams& p, const cf* tw, const int* done, int num_sms, cudaStream_t st) {
-    int nb = 1;
-    size_t smem = 0;
-    cudaError_t e;
-    switch (merged_group(p.S2)) {
-        case 1:
-            if ((e = merged_grid<1>(p.t, p.n_lines, num_sms, &nb, &smem)) != cudaSuccess) return e;
-            k_line_merged<1><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
-            break;
-        case 2:
-            if ((e = merged_grid<2>(p.t, p.n_lines, num_sms, &nb, &smem)) != cudaSuccess) return e;
-            k_line_merged<2><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
-            break;
-        case 4:
-            if ((e = merged_grid<4>(p.t, p.n_lines, num_sms, &nb, &smem)) != cudaSuccess) return e;
-            k_line_merged<4><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
-            break;
-        case 8:
-            if ((e = merged_grid<8>(p.t, p.n_lines, num_sms, &nb, &smem)) != cudaSuccess) return e;
-            k_line_merged<8><<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
-            break;
-        default: return cudaErrorNotSupported;
-    }
-    return cudaGetLastError();
-}
-
-// grid size of the merged sweep (= number of residual partials it writes); 0 if the shape does not allow merging
-int merged_blocks_entry(int S2, int t, long long n_lines, int num_sms) {
-    int nb = 0;
-    size_t smem = 0;
-    cudaError_t e = cudaErrorNotSupported;
-    switch (merged_group(S2)) {
-        case 1: e = merged_grid<1>(t, n_lines, num_sms, &nb, &smem); break;
-        case 2: e = merged_grid<2>(t, n_lines, num_sms, &nb, &smem); break;
-        case 4: e = merged_grid<4>(t, n_lines, num_sms, &nb, &smem); break;
-        case 8: e = merged_grid<8>(t, n_lines, num_sms, &nb, &smem); break;
-        default: return 0;
-    }
-    return e == cudaSuccess ? nb : 0;
-}
-
 int line_blocks_entry(int mode, int t, int variant, long long n_lines, int num_sms) {
     int nb = 1;
     size_t smem = 0;
@@ -424,7 +336,6 @@ cudaError_t contig_entry(const cf* src, cf* dst, const ContigGeom& g, const Symb
 extern const FftEntry MBS_CAT(g_fft_entry_, MBS_FFT_SIZE) = {
     MBS_FFT_SIZE, CS, CSM, CC, strided_entry, contig_entry, fused_ok() ? fused_entry : nullptr,
     fused_ok() ? fused_blocks_entry : nullptr,
-    line_ok() ? line_entry : nullptr, line_ok() ? line_blocks_entry : nullptr,
-    line_ok() ? merged_entry : nullptr, line_ok() ? merged_blocks_entry : nullptr};
+    line_ok() ? line_entry : nullptr, line_ok() ? line_blocks_entry : nullptr};
 
 }  // namespace mbs

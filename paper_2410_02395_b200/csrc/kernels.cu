@@ -353,172 +353,6 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
     grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, p.finish, RED_RESIDUAL, p.state, p.hist, red);
 }
 
-// ---------------------------------------------------------------------------------------------
-// All slab passes in ONE launch (MBS_OPT_SLAB_FUSED).  Blocks [0, nb0) take the items of axis 0, [nb0, nb0 + nb1) those of
-// axis 1, the rest those of axis 2 (an axis without corrections has no blocks).  Instead of handing a voxel that is an edge
-// point of several axes from pass to pass through u, every slab voxel has one owner -- the item of the LOWEST axis on which
-// it is an edge point -- and the owner applies all its corrections: corr of its own axis as in k_slab_pass (t outputs from
-// 2t values), and for the few voxels that are also edge points of a higher axis b the value corr_b(d) at that voxel,
-// gathered from the compact d of axis b (2t loads).  Items of a higher axis skip the lines an earlier axis owns.
-// ---------------------------------------------------------------------------------------------
-struct SlabAllParams {
-    const cf* ds[3];
-    const cf* u;
-    cf* x;
-    const float* Kh;
-    cf c;
-    int e[3];          // axis has edge corrections
-    float alpha;
-    double* partials;
-    int slot0;
-    DevState* state;
-    double* hist;
-    const int* active;
-    unsigned nb0, nb1; // block ranges
-};
-
-// corr_b(d) at ONE voxel that is an edge point of axis b: slot = s*2t + e (first t: e < t; last t: e >= t) of that axis;
-// dsb + base + q * qstride walks the compact d of the line through the voxel (q = slot index along the axis)
-template <int TT>
-__device__ __forceinline__ cf slab_gather_corr(const GridDesc& g, const cf* dsb, const long long base, const long long qstride,
-                                               const int b, const int slot, const float* Ks, const cf c) {
-    const int S = g.S[b];
-    const int s = slot / (2 * TT), e = slot - s * 2 * TT;
-    const bool last = e >= TT;
-    const int k = last ? e - TT : e;
-    int nb = last ? s + 1 : s - 1;
-    bool has_nb = true;
-    if (nb < 0 || nb >= S) {
-        if (g.per[b]) nb = (nb + S) % S;
-        else has_nb = false;
-    }
-    // last edge reads the FIRST t points of s and s+1; first edge reads the LAST t points of s and s-1
-    const cf* own = dsb + base + (long long)(s * 2 * TT + (last ? 0 : TT)) * qstride;
-    const cf* nbp = dsb + base + (long long)(nb * 2 * TT + (last ? 0 : TT)) * qstride;
-    float sr = 0.f, si = 0.f;
-#pragma unroll 2
-    for (int q = 0; q < TT; ++q) {
-        const cf ov = own[q * qstride];
-        cf nv = make_float2(0.f, 0.f);
-        if (has_nb) nv = nbp[q * qstride];
-        const float kk = last ? Ks[k * TT + q] : Ks[q * TT + k];
-        sr = fmaf(kk, nv.x - ov.x, sr);
-        si = fmaf(kk, nv.y - ov.y, si);
-    }
-    return cmul(c, make_float2(sr, si));
-}
-
-// the items of axis AX (compile-time, so that the grid description is indexed statically), spread over `nblocks` blocks
-template <int TT, bool ACT, int AX>
-__device__ __forceinline__ float slab_all_axis(const GridDesc& g, const SlabAllParams& p, const float* Ks, const unsigned block,
-                                               const unsigned nblocks) {
-    constexpr int t = TT;
-    const int S = g.S[AX], M = g.M[AX];
-    const unsigned N1 = (unsigned)g.N[1], N2 = (unsigned)g.N[2];
-    const unsigned outer = AX == 0 ? 1u : (AX == 1 ? (unsigned)g.N[0] : (unsigned)g.N[0] * N1);
-    const unsigned inner = AX == 0 ? N1 * N2 : (AX == 1 ? N2 : 1u);
-    const unsigned n_items = outer * (unsigned)S * 2u * inner;          // < 2^31 (mbs_create)
-    const int E1 = g.S[1] * 2 * t, E2 = g.S[2] * 2 * t;
-    const cf* __restrict__ ds = p.ds[AX];
-    float acc = 0.f;
-    for (unsigned item = block * SLAB_THREADS + threadIdx.x; item < n_items; item += nblocks * SLAB_THREADS) {
-        const unsigned rest0 = item / inner;
-        const unsigned in_i = item - rest0 * inner;
-        const int side = (int)(rest0 & 1u);
-        const unsigned rest1 = rest0 >> 1;
-        const unsigned o = rest1 / (unsigned)S;
-        const int s = (int)(rest1 - o * (unsigned)S);
-        // grid indices of the item's line (the index along AX varies over its t outputs), ownership, extra axes
-        int i0 = 0, i1 = 0, i2 = 0, q1 = -1, q2 = -1;
-        if constexpr (AX == 0) {
-            i1 = (int)(in_i / N2); i2 = (int)(in_i - (unsigned)i1 * N2);
-            if (p.e[1]) q1 = edge_slot(i1, g.M[1], t);
-            if (p.e[2]) q2 = edge_slot(i2, g.M[2], t);
-        } else if constexpr (AX == 1) {
-            i0 = (int)o; i2 = (int)in_i;
-            if (p.e[0] && edge_slot(i0, g.M[0], t) >= 0) continue;      // the line belongs to an axis-0 item
-            if (p.e[2]) q2 = edge_slot(i2, g.M[2], t);
-        } else {
-            i0 = (int)(o / N1); i1 = (int)(o - (unsigned)i0 * N1);
-            if ((p.e[0] && edge_slot(i0, g.M[0], t) >= 0) || (p.e[1] && edge_slot(i1, g.M[1], t) >= 0)) continue;
-        }
-        if constexpr (ACT) {
-            int s0, s1, s2;
-            if constexpr (AX == 0) { s0 = s; s1 = i1 / g.M[1]; s2 = i2 / g.M[2]; }
-            else if constexpr (AX == 1) { s0 = i0 / g.M[0]; s1 = s; s2 = i2 / g.M[2]; }
-            else { s0 = i0 / g.M[0]; s1 = i1 / g.M[1]; s2 = s; }
-            if (!p.active[(s0 * g.S[1] + s1) * g.S[2] + s2]) continue;
-        }
-        int nb = side ? s + 1 : s - 1;
-        bool has_nb = true;
-        if (nb < 0 || nb >= S) {
-            if (g.per[AX]) nb = (nb + S) % S;
-            else has_nb = false;
-        }
-        // side 1 (last t points of s) reads the FIRST t points of s and s+1; side 0 reads the LAST t points
-        const long long own0 = ((long long)(o * (unsigned)S + (unsigned)s) * 2 * t + (side ? 0 : t)) * inner + in_i;
-        const long long nb0 = ((long long)(o * (unsigned)S + (unsigned)nb) * 2 * t + (side ? 0 : t)) * inner + in_i;
-        cf dv[TT];
-#pragma unroll
-        for (int q = 0; q < TT; ++q) {
-            const cf own = ds[own0 + (long long)q * inner];
-            cf nbv = make_float2(0.f, 0.f);
-            if (has_nb) nbv = ds[nb0 + (long long)q * inner];
-            dv[q] = make_float2(nbv.x - own.x, nbv.y - own.y);
-        }
-        const int ia0 = s * M + (side ? M - t : 0);     // first output index along AX
-        long long vox0, vstride;
-        if constexpr (AX == 0) { vox0 = (long long)ia0 * inner + in_i; vstride = inner; }
-        else if constexpr (AX == 1) { vox0 = ((long long)o * N1 + ia0) * inner + in_i; vstride = inner; }
-        else { vox0 = (long long)o * N2 + ia0; vstride = 1; }
-        const bool multi = (q1 >= 0) || (q2 >= 0);      // also an edge point of a higher axis (a few per cent of the items)
-#pragma unroll
-        for (int e = 0; e < TT; ++e) {
-            float sr = 0.f, si = 0.f;
-#pragma unroll
-            for (int q = 0; q < TT; ++q) {
-                const float k = side ? Ks[e * TT + q] : Ks[q * TT + e];
-                sr = fmaf(k, dv[q].x, sr);
-                si = fmaf(k, dv[q].y, si);
-            }
-            const cf corr = cmul(p.c, make_float2(sr, si));
-            const long long vox = vox0 + e * vstride;
-            const cf uu = p.u[vox];
-            cf r = make_float2(uu.x - corr.x, uu.y - corr.y);
-            if (multi) {
-                if (q1 >= 0) {                                          // (AX == 0) also an edge point of axis 1
-                    const cf c1 = slab_gather_corr<TT>(g, p.ds[1], (long long)(ia0 + e) * E1 * N2 + i2, (long long)N2, 1, q1, Ks, p.c);
-                    r = make_float2(r.x - c1.x, r.y - c1.y);
-                }
-                if (q2 >= 0) {                                          // also an edge point of axis 2
-                    const int j0 = AX == 0 ? ia0 + e : i0, j1 = AX == 1 ? ia0 + e : i1;
-                    const cf c2 = slab_gather_corr<TT>(g, p.ds[2], ((long long)j0 * N1 + j1) * E2, 1LL, 2, q2, Ks, p.c);
-                    r = make_float2(r.x - c2.x, r.y - c2.y);
-                }
-            }
-            const cf xv = p.x[vox];
-            acc += r.x * r.x + r.y * r.y;
-            p.x[vox] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
-        }
-    }
-    return acc;
-}
-
-template <int TT, bool ACT>
-__global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_all(const GridDesc g, const SlabAllParams p) {
-    __shared__ float Ks[TT * TT];
-    __shared__ double red[32];
-    if (p.state->done) return;
-    for (int i = threadIdx.x; i < TT * TT; i += SLAB_THREADS) Ks[i] = p.Kh[i];
-    __syncthreads();
-    float acc;
-    if (blockIdx.x < p.nb0) acc = slab_all_axis<TT, ACT, 0>(g, p, Ks, blockIdx.x, p.nb0);
-    else if (blockIdx.x < p.nb0 + p.nb1) acc = slab_all_axis<TT, ACT, 1>(g, p, Ks, blockIdx.x - p.nb0, p.nb1);
-    else acc = slab_all_axis<TT, ACT, 2>(g, p, Ks, blockIdx.x - p.nb0 - p.nb1, gridDim.x - p.nb0 - p.nb1);
-    const double bs = block_sum((double)acc, red);
-    grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, 1, RED_RESIDUAL, p.state, p.hist, red);
-}
-
 int slab_pass_blocks(const GridDesc& g, int ax) {
     long long outer = 1, inner = 1;
     for (int d = 0; d < ax; ++d) outer *= g.N[d];
@@ -549,35 +383,6 @@ cudaError_t launch_slab_pass(const GridDesc& g, const SlabPassParams& p, cudaStr
         default: return cudaErrorNotSupported;
     }
 #undef MBS_SLAB_PASS
-    return cudaGetLastError();
-}
-
-int slab_pass_all_blocks(const GridDesc& g, int mask) {
-    int n = 0;
-    for (int ax = 0; ax < 3; ++ax)
-        if ((mask >> ax) & 1) n += slab_pass_blocks(g, ax);
-    return n;
-}
-
-cudaError_t launch_slab_pass_all(const GridDesc& g, const SlabPassParams& p0, const cf* const ds[3], int mask, cudaStream_t st) {
-    SlabAllParams p{};
-    for (int ax = 0; ax < 3; ++ax) { p.ds[ax] = ds[ax]; p.e[ax] = (mask >> ax) & 1; }
-    p.u = p0.u; p.x = p0.x; p.Kh = p0.Kh; p.c = p0.c; p.alpha = p0.alpha; p.partials = p0.partials; p.slot0 = p0.slot0;
-    p.state = p0.state; p.hist = p0.hist; p.active = p0.active;
-    p.nb0 = p.e[0] ? (unsigned)slab_pass_blocks(g, 0) : 0u;
-    p.nb1 = p.e[1] ? (unsigned)slab_pass_blocks(g, 1) : 0u;
-    const unsigned nb = (unsigned)slab_pass_all_blocks(g, mask);
-#define MBS_SLAB_ALL(TTv)                                                              \
-    if (p.active) k_slab_pass_all<TTv, true><<<nb, SLAB_THREADS, 0, st>>>(g, p);       \
-    else k_slab_pass_all<TTv, false><<<nb, SLAB_THREADS, 0, st>>>(g, p)
-    switch (g.t) {
-        case 2: MBS_SLAB_ALL(2); break;
-        case 4: MBS_SLAB_ALL(4); break;
-        case 8: MBS_SLAB_ALL(8); break;
-        case 16: MBS_SLAB_ALL(16); break;
-        default: return cudaErrorNotSupported;
-    }
-#undef MBS_SLAB_ALL
     return cudaGetLastError();
 }
 

@@ -82,10 +82,6 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
         if (!in_range) line = n_lines - 1;            // clamp: loads stay legal, stores are masked
         unsigned row = line / (unsigned)p.S2;
         const int seg = (int)(line - row * (unsigned)p.S2);
-        if (MODE == LINE_S1 && p.slab_rows_only) {
-            row = line_slab_row(p, row);
-            line = row * (unsigned)p.S2 + (unsigned)seg;
-        }
         const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
         bool valid = in_range;
         if constexpr (ACT) {
@@ -144,7 +140,7 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
                 if (last_edge) v[P - 1] = csub(v[P - 1], fast_corr2_x<M, TT>(p, Ks, grow, seg, true, k_last));
             }
 #ifndef MBS_NO_L2_PREFETCH
-            if (!p.slab_rows_only) {
+            {
                 const unsigned nline = (unit + gridDim.x * NWARP) * LW + lsub;
                 bool want = nline < n_lines;
                 if constexpr (ACT) {

@@ -108,31 +108,6 @@ __device__ __forceinline__ int line_edge_index(int q, int M, int t) {   // q in 
     return s * M + (e < t ? e : M - 2 * t + e);
 }
 
-// k-th row (in the enumeration of k_fixup: set A = {i0 edge of axis 0} x all i1, then set B = {i0 not an edge of
-// axis 0} x {i1 edge of axis 1}) -> row index i0 * N1 + i1
-__device__ __forceinline__ unsigned line_slab_row(const FusedParams& p, unsigned rid) {
-    const int t = p.t;
-    const unsigned nE0 = p.e0 ? (unsigned)(p.S0 * 2 * t) : 0u, nE1 = p.e1 ? (unsigned)(p.S1 * 2 * t) : 0u;
-    const unsigned rowsA = nE0 * (unsigned)p.N1;
-    int i0, i1;
-    if (rid < rowsA) {
-        const unsigned q0 = rid / (unsigned)p.N1;
-        i1 = (int)(rid - q0 * (unsigned)p.N1);
-        i0 = line_edge_index((int)q0, p.M0, t);
-    } else {
-        const unsigned rb = rid - rowsA;
-        const unsigned k0 = rb / nE1;
-        i1 = line_edge_index((int)(rb - k0 * nE1), p.M1, t);
-        if (p.e0) {
-            const int w = p.M0 - 2 * t, s = (int)k0 / w;
-            i0 = s * p.M0 + t + ((int)k0 - s * w);
-        } else {
-            i0 = (int)k0;
-        }
-    }
-    return (unsigned)i0 * (unsigned)p.N1 + (unsigned)i1;
-}
-
 // ACT: subdomain activation -- lines of inactive subdomains are skipped; a separate instantiation so that
 // the plain kernels keep their code exactly
 template <class PL, int NWARP, int MODE, bool ACT = false>
@@ -161,10 +136,6 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
         const bool in_range = line < n_lines;
         unsigned row = line / (unsigned)p.S2;
         const int seg = (int)(line - row * (unsigned)p.S2);
-        if (MODE == LINE_S1 && p.slab_rows_only) {    // `line` counted slab-row lines: map to the real row
-            row = in_range ? line_slab_row(p, row) : 0u;
-            line = row * (unsigned)p.S2 + (unsigned)seg;
-        }
         const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
         bool act_ok = true;
         if constexpr (ACT) {
@@ -220,7 +191,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
 #ifndef MBS_NO_L2_PREFETCH
             // x and B_diag of the line this warp takes next are requested into L2 now (one 128-byte line per lane and
             // request: no registers, no shared memory), so that their loads after this FFT are L2 hits
-            if (!p.slab_rows_only) {
+            {
                 const unsigned nline = (unit + gridDim.x * NWARP) * LW + lsub;
                 bool want = nline < n_lines;
                 if constexpr (ACT) {

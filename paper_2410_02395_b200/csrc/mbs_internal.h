@@ -127,10 +127,6 @@ struct SlabPassParams {
 int slab_pass_blocks(const GridDesc& g, int ax);
 bool slab_pass_supported(int t);
 cudaError_t launch_slab_pass(const GridDesc& g, const SlabPassParams& p, cudaStream_t st);
-// all axes of `mask` in one launch (k_slab_pass_all): p.ds / p.axis / p.e1 / p.e2 / p.finish of `p` are not used; the
-// launch writes slab_pass_all_blocks(g, mask) partials from p.slot0 on and finishes the iteration
-int slab_pass_all_blocks(const GridDesc& g, int mask);
-cudaError_t launch_slab_pass_all(const GridDesc& g, const SlabPassParams& p, const cf* const ds[3], int mask, cudaStream_t st);
 int fixup_blocks(const GridDesc& g, int e0, int e1, int e2, int num_sms);
 cudaError_t launch_fixup(const GridDesc& g, const FixupParams& p, int nblocks, cudaStream_t st);
 cudaError_t launch_row_mask(const cf* y, unsigned char* mask, long long rows, int N2, cudaStream_t st);
@@ -152,7 +148,7 @@ cudaError_t launch_setup(const GridDesc& g, const SetupParams& p, int pass, doub
 
 // fused first / last sweep along the contiguous axis (fused_kernels.cuh)
 enum FusedMode { FUSED_S1 = 0, FUSED_S5 = 1, FUSED_1D = 2 };
-enum LineMode { LINE_S1 = 0, LINE_S5 = 1, LINE_S51 = 2 };   // warp-line variant (line_kernels.cuh)
+enum LineMode { LINE_S1 = 0, LINE_S5 = 1 };   // warp-line variant (line_kernels.cuh)
 
 struct FusedParams {
     cf* x;               // iterate: read by S1; read and updated in place by S5 / 1D
@@ -163,7 +159,6 @@ struct FusedParams {
     cf* u;               // S1: output; S5: input u' lines, output r_part on slab rows
     int N0, N1, N2;      // grid extents (N2 = S2 * M)
     int S0;              // subdomains along axis 0
-    int slab_rows_only;  // warp-line sweep 1: visit only the rows that lie in a slab of axis 0 or 1 (n_lines counts those)
     int S2, a2, per2;    // subdomains, a_d and periodic flag of the last axis
     int t;               // correction points
     int e0, e1;          // 1 if axis 0 / 1 has edge corrections
@@ -229,10 +224,6 @@ struct FftEntry {
     // warp-line variant of the first / last sweep (line_kernels.cuh); nullptr when a line does not fit in a warp
     cudaError_t (*line)(const FusedParams& p, const cf* tw, int mode, const int* done, int num_sms, cudaStream_t st);
     int (*line_blocks)(int mode, int t, int variant, long long n_lines, int num_sms);   // variant: FusedParams::line_variant
-    // last sweep merged with the next iteration's first sweep (line_merged.cuh); merged_blocks = grid size, 0 if the
-    // number of subdomains along the last axis does not map onto whole warps of one CTA
-    cudaError_t (*merged)(const FusedParams& p, const cf* tw, const int* done, int num_sms, cudaStream_t st);
-    int (*merged_blocks)(int S2, int t, long long n_lines, int num_sms);
 };
 const FftEntry* fft_lookup(int M);
 

@@ -211,11 +211,11 @@ ITERATION_CASES = OPERATOR_CASES + [
 ]
 
 
-# kernel variants: merged sweep; default (warp-line kernels, compile-time-t variant where it is used); warp-line generic only;
-# tile kernels; one kernel per step; no TMA
-@pytest.mark.parametrize("fused,tma,line,merge", [(1, 1, 1, 1), (1, 1, 1, 0), (1, 1, 2, 0), (1, 1, 0, 0), (0, 1, 1, 0), (1, 0, 0, 0)])
+# kernel variants: default (warp-line kernels, compile-time-t variant where it is used); warp-line generic only; tile kernels;
+# one kernel per step; no TMA
+@pytest.mark.parametrize("fused,tma,line", [(1, 1, 1), (1, 1, 2), (1, 1, 0), (0, 1, 1), (1, 0, 0)])
 @pytest.mark.parametrize("shape,S,W,t,periodic", ITERATION_CASES)
-def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line, merge):
+def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line):
     """A few updates of Eq. (6) from a random start with a dense random source, fused sweeps and
     one-kernel-per-step path, against the oracle's iterates: every step of SURVEY 8(a) on every geometry."""
     import torch
@@ -223,7 +223,6 @@ def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line, me
     s.set_option(B.MBS_OPT_FUSED, fused)
     s.set_option(B.MBS_OPT_TMA, tma)
     s.set_option(B.MBS_OPT_LINE, line)
-    s.set_option(B.MBS_OPT_MERGE, merge)
     y = workloads.random_field(shape, 21)
     x0 = workloads.random_field(shape, 22)
     n_it = 6
@@ -237,24 +236,6 @@ def test_iteration_parity(B, orc, shape, S, W, t, periodic, fused, tma, line, me
     x2, hist2, rc = s.solve(y, x0=x0, tol=0.0, max_iter=n_it)
     assert rc == B.MBS_ERR_NOT_CONVERGED
     assert np.array_equal(hist2, hist) and torch.equal(x2, xd)
-    s.close()
-
-
-@pytest.mark.parametrize("shape,S,W,t,periodic", [c for c in ITERATION_CASES if len(c[0]) >= 2])
-def test_iteration_parity_slab_passes_in_one_launch(B, orc, shape, S, W, t, periodic):
-    """MBS_OPT_SLAB_FUSED: the slab passes of all axes as one launch in which every slab voxel has one owner."""
-    import torch
-    s, o, n = make_pair(B, orc, shape, S, W, t, periodic, seed=11)
-    s.set_option(B.MBS_OPT_SLAB_FUSED, 1)
-    y = workloads.random_field(shape, 21)
-    x0 = workloads.random_field(shape, 22)
-    n_it = 6
-    x_ref, h_ref = cached(("iter", shape, S, W, t, periodic), lambda: o.solve(y, x0=x0, tol=0.0, max_iter=n_it))
-    yd = torch.from_numpy(y).cuda()
-    xd = torch.from_numpy(x0).cuda()
-    hist = s.iterate(yd, xd, n_it)
-    assert np.allclose(hist, h_ref, rtol=2e-5), (hist, h_ref)
-    check_field(xd.cpu().numpy(), x_ref, OP_TOL, shape, S, t, periodic, what="iterate, slab passes in one launch")
     s.close()
 
 
