@@ -69,7 +69,7 @@ def build(force: bool = False, verbose: bool = False, sizes=None) -> str:
     `sizes` (kernel development only: `--sizes 256,512`) links a library that knows just those subdomain lengths."""
     os.makedirs(OBJDIR, exist_ok=True)
     jobs = []
-    for name in ("api.cu", "kernels.cu"):
+    for name in ("api.cu", "kernels.cu", "refine_f64.cu"):
         jobs.append((os.path.join(CSRC, name), os.path.join(OBJDIR, name[:-3] + ".o"), []))
     if sizes:
         tag = "_".join(str(m) for m in sizes)

@@ -94,6 +94,10 @@ struct mbs_ctx {
     int refine = -1;                 // MBS_OPT_REFINE: -1 automatic (grids of <= 2^21 voxels), 0 off, 1 on
     cf* delta = nullptr;             // owned: the small part of the iterate
     cf* dref = nullptr;              // owned: d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec)
+    double* bdiag64 = nullptr;       // owned: B_diag in complex128 (grids that may use the split iterate)
+    double* Kh64_dev = nullptr;      // owned: K_t / h^2 in double
+    double* tw64_dev[3] = {nullptr, nullptr, nullptr};   // owned: double twiddle tables per axis
+    double* f64buf[2] = {nullptr, nullptr};              // owned: complex128 work arrays
     bool split = false;              // the running solve iterates on delta
     double split_eps = 1.0;          // eps at the last re-centering
     int n_recenter = 0;
@@ -434,6 +438,10 @@ extern "C" void mbs_destroy(mbs_ctx* c) {
     if (c->act_mem) cudaFree(c->act_mem);
     if (c->delta) cudaFree(c->delta);
     if (c->dref) cudaFree(c->dref);
+    if (c->bdiag64) cudaFree(c->bdiag64);
+    if (c->Kh64_dev) cudaFree(c->Kh64_dev);
+    for (int i = 0; i < 3; ++i) if (c->tw64_dev[i]) cudaFree(c->tw64_dev[i]);
+    for (int i = 0; i < 2; ++i) if (c->f64buf[i]) cudaFree(c->f64buf[i]);
     delete c;
 }
 
@@ -520,6 +528,9 @@ extern "C" int mbs_get_activation(const mbs_ctx* c, int32_t* activated_at, int32
 // ---------------------------------------------------------------------------------------------
 // set_potential (a0 of the scope table)
 // ---------------------------------------------------------------------------------------------
+// grids on which the split iterate may run (small, L2-resident: configs 1 and 2) get the double-precision tables
+static bool split_grid(const mbs_ctx* c) { return c->refine == 1 || (c->refine < 0 && c->g.voxels <= (1LL << 21)); }
+
 extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
     if (!c) return MBS_ERR_INVALID_ARG;
     if (!n_map_device) return fail(c, MBS_ERR_INVALID_ARG, "n_map is NULL");
@@ -563,6 +574,8 @@ extern "C" int mbs_set_potential(mbs_ctx* c, const void* n_map_device) {
     c->c = cd(0.0, -0.95 / denom);
     sp.c_re = c->c.real();
     sp.c_im = c->c.imag();
+    if (split_grid(c) && !c->bdiag64) MBS_CUDA(c, cudaMalloc(&c->bdiag64, 2 * sizeof(double) * (size_t)g.voxels));
+    sp.bdiag64 = c->bdiag64;
     { KernelScope ks(c, "setup_bdiag", 2 * vb); MBS_CUDA(c, launch_setup(g, sp, 2, nullptr, c->bdiag, nblocks, c->stream)); }
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));
     c->potential_set = true;
@@ -882,9 +895,57 @@ static bool split_effective(const mbs_ctx* c) {
     return want && c->fused && fused_available(c) && !c->activation;
 }
 
+// double tables and work arrays of refine_f64.cu (once per context)
+static int ensure_f64_tables(mbs_ctx* c) {
+    const GridDesc& g = c->g;
+    if (!c->Kh64_dev && g.t > 0) {
+        MBS_CUDA(c, cudaMalloc(&c->Kh64_dev, sizeof(double) * c->Kh.size()));
+        MBS_CUDA(c, cudaMemcpy(c->Kh64_dev, c->Kh.data(), sizeof(double) * c->Kh.size(), cudaMemcpyHostToDevice));
+    }
+    for (int ax = c->first; ax < 3; ++ax) {
+        if (c->tw64_dev[ax]) continue;
+        const int M = g.M[ax];
+        std::vector<double> tw(2 * (size_t)M);
+        for (int n = 0; n < M; ++n) {
+            const double ang = 2.0 * M_PI * (double)n / (double)M;
+            tw[2 * n] = cos(ang);
+            tw[2 * n + 1] = -sin(ang);
+        }
+        MBS_CUDA(c, cudaMalloc(&c->tw64_dev[ax], sizeof(double) * tw.size()));
+        MBS_CUDA(c, cudaMemcpy(c->tw64_dev[ax], tw.data(), sizeof(double) * tw.size(), cudaMemcpyHostToDevice));
+    }
+    for (int i = 0; i < 2; ++i)
+        if (!c->f64buf[i]) MBS_CUDA(c, cudaMalloc(&c->f64buf[i], 2 * sizeof(double) * (size_t)g.voxels));
+    return MBS_OK;
+}
+
 static int recenter(mbs_ctx* c, const cf* y, cf* x, bool add_delta) {
     const size_t bytes = sizeof(cf) * (size_t)c->g.voxels;
     const double vb = 8.0 * (double)c->g.voxels;
+    if (c->bdiag64) {
+        // mixed-precision refinement: the residual of the frozen part in complex128 (refine_f64.cu)
+        if (add_delta) {                                      // x_ref <- x_ref + delta
+            PointwiseParams p = pw_defaults(c, false);
+            p.in = x; p.w = c->delta; p.s1 = 1.f; p.s2 = 1.f; p.out = x;
+            KernelScope ks(c, "recenter_add", 3 * vb);
+            MBS_CUDA(c, launch_pointwise(c->g, p, c->num_sms, c->stream));
+        }
+        MBS_TRY(ensure_f64_tables(c));
+        RefineF64 r{};
+        r.bdiag = c->bdiag64; r.Kh = c->Kh64_dev;
+        for (int ax = 0; ax < 3; ++ax) r.tw[ax] = c->tw64_dev[ax];
+        r.buf[0] = c->f64buf[0]; r.buf[1] = c->f64buf[1];
+        r.c_re = c->c.real(); r.c_im = c->c.imag(); r.k02_re = c->k02.real(); r.k02_im = c->k02.imag(); r.h = c->h;
+        r.first_axis = c->first;
+        {
+            KernelScope ks(c, "recenter_dref_f64", 3 * vb);
+            c->launches += 2 * c->ndim + 2;                   // (the scope counted one of the 2 ndim + 3 launches)
+            MBS_CUDA(c, launch_dref_f64(c->g, r, x, y, c->dref, c->stream));
+        }
+        MBS_CUDA(c, cudaMemsetAsync(c->delta, 0, bytes, c->stream));
+        c->n_recenter++;
+        return MBS_OK;
+    }
     if (add_delta) {                                          // x_ref <- x_ref + delta
         PointwiseParams p = pw_defaults(c, false);
         p.in = x; p.w = c->delta; p.s1 = 1.f; p.s2 = 1.f; p.out = x;
@@ -1076,14 +1137,22 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
             pending[prev] = false;
             const DevState& st = c->state_pinned[prev];
             if (st.done) { final_done = st.done; break; }
-            if (c->split && st.iter > 0 && st.nu2 > 0 && c->n_recenter < 16) {
-                // split iterate: re-centre each time the residual has dropped by an order of magnitude (what is enqueued
-                // here runs after the batch already in flight; in exact arithmetic it changes nothing).  A re-centring
-                // draws a fresh fp32 rounding of (L+I)^-1 (B x_ref + y_vec), a one-off perturbation of the size of the
-                // plain complex64 floor, about 2.4e-7 ||x|| / nu: it is done only while eps is 30 x above it.
+            if (c->split && st.iter > 0 && st.nu2 > 0 && c->n_recenter < 64) {
+                // split iterate: re-centre as the residual falls (what is enqueued here runs after the batch already in
+                // flight; in exact arithmetic it changes nothing).  With the double-precision residual (bdiag64) every
+                // re-centring removes the complex64 rounding accumulated in delta: once per factor 2 of the residual.  The
+                // complex64 fallback draws a fresh fp32 rounding of (L+I)^-1 (B x_ref + y_vec) each time, a one-off
+                // perturbation of the size of the plain floor, about 2.4e-7 ||x|| / nu: once per decade and
+                // only while eps is 30 x above that floor.
                 const double eps = sqrt(st.last_sum / st.nu2);
-                const double floor_plain = 2.4e-7 * sqrt(st.xnorm2 / st.nu2);
-                if (eps < 0.1 * c->split_eps && eps > 30.0 * floor_plain) {
+                bool go;
+                if (c->bdiag64) {
+                    go = eps < 0.5 * c->split_eps;
+                } else {
+                    const double floor_plain = 2.4e-7 * sqrt(st.xnorm2 / st.nu2);
+                    go = eps < 0.1 * c->split_eps && eps > 30.0 * floor_plain;
+                }
+                if (go) {
                     MBS_TRY(recenter(c, y, x, true));
                     c->split_eps = eps;
                 }

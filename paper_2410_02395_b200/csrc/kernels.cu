@@ -882,6 +882,7 @@ __global__ void __launch_bounds__(256) k_setup(const GridDesc g, const SetupPara
                 const double br = 1.0 - (p.c_re * dr - p.c_im * di);
                 const double bi = -(p.c_re * di + p.c_im * dr);
                 bdiag[idx] = make_float2((float)br, (float)bi);
+                if (p.bdiag64) { p.bdiag64[2 * idx] = br; p.bdiag64[2 * idx + 1] = bi; }
             }
         }
     }

@@ -139,6 +139,7 @@ struct SetupParams {
     int W[3];
     double k02_re, k02_im;
     double c_re, c_im;
+    double* bdiag64;     // optional (pass 2): B_diag also as complex128 (interleaved re, im) for refine_f64.cu
 };
 // pass 0: per-block min/max of Re k^2, Im k^2 and min Im n -> out[block*5 + {0..4}]
 // pass 1: per-block max |k^2 - k0^2|^2                     -> out[block]
@@ -207,6 +208,18 @@ cudaError_t launch_activation_init(const GridDesc& g, const ActivationState& a, 
 cudaError_t launch_activation_step(const GridDesc& g, const ActivationState& a, const cf* x, const float* Kh, cf c,
                                    DevState* state, cudaStream_t st);
 
+
+// Double-precision residual of the frozen part of the split iterate (refine_f64.cu): everything the kernels need.
+struct RefineF64 {
+    const double* bdiag;   // B_diag as complex128 (interleaved)
+    const double* Kh;      // K_t / h^2, t x t row-major, double
+    const double* tw[3];   // per axis: exp(-2 pi i j / M_d), j in [0, M_d), complex128 (interleaved); nullptr for unit axes
+    double* buf[2];        // two complex128 work arrays of the grid size
+    double c_re, c_im, k02_re, k02_im, h;
+    int first_axis;        // first real axis of the internal 3-D description
+};
+// dref = x - (L+I)^-1 (B x + y_vec) evaluated in complex128, rounded once to complex64 (y may be nullptr)
+cudaError_t launch_dref_f64(const GridDesc& g, const RefineF64& r, const cf* x, const cf* y, cf* dref, cudaStream_t st);
 
 // FFT registry (fft_inst.cu compiled once per size, fft_registry.cu)
 struct FftEntry {
