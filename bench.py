@@ -449,7 +449,8 @@ def main():
     if args.config is None and shape is None and not args.no_other_configs:
         others = []
         for oc in (3, 4):
-            so, wo, yo, xo, ro = time_config(oc, args.steps if args.steps is not None else DEFAULT_STEPS[oc], W, dev, world)
+            # their own window (at least 50 iterations where an iteration is short), not the primary's K
+            so, wo, yo, xo, ro = time_config(oc, DEFAULT_STEPS[oc], W, dev, world)
             so.close()
             del so, yo, xo
             torch.cuda.empty_cache()

@@ -21,6 +21,7 @@ Readings of points the paper leaves open (listed in DESIGN.md section 3, after S
   R8  eps_n belongs to x^(n); the update is applied before the stop test.
   R9  p = 2 pi fftfreq(M, h); forward unnormalised, inverse 1/M.
   R17 subdomain activation (the paper gives neither the norm nor the threshold): see solve_activated.
+  R18 batched solves ("solving each frequency separately"; several sources sharing one medium): see solve_batch.
 
 Pins (tests/test_oracle_pins.py, `-m "not gpu"`): printed K_t / sigma_max values, Eq. (9) -> Eq. (4),
 dense assembly from explicit DFT matrices, dense direct solve, monotone residual, eps_0 = 1,
@@ -287,6 +288,35 @@ def solve_activated(o, y, x0=None, tol=1e-6, max_iter=1000, threshold=None, call
         if eps < tol:
             break
     return x, np.asarray(history), activated_at
+
+
+# ---- batched solves: several sources, one medium, reading R18 -----------------------------------
+def solve_batch(o, ys, x0s=None, tol=1e-6, max_iter=1000):
+    """Several right-hand sides y_b for one medium and wavelength (time- or source-dependent problems are solved
+    "separately", one system per source; they share A).  Reading R18: the sources are iterated in
+    lock step with Eq. (6), each exactly as `solve` would, and ONE stop test is applied to the stacked system
+    diag(A, ..., A) [x_1 ... x_B] = [y_1 ... y_B], whose relative residual is
+        eps_n = sqrt( sum_b ||r_b^(n)||^2 ) / sqrt( sum_b ||Gamma^-1 y_vec,b||^2 ).
+    Nothing couples the sources: x_b^(n) equals the n-th iterate of `solve(y_b)`.
+    Returns (list of fields, residual_history of the stacked system)."""
+    ys = [np.asarray(y).astype(np.complex128) for y in ys]
+    y_vecs = [-o.c * y for y in ys]
+    xs = [np.zeros(o.shape, dtype=np.complex128) if x0s is None else np.asarray(x0).astype(np.complex128).copy()
+          for x0 in (x0s if x0s is not None else ys)]
+    nu2 = sum(np.linalg.norm(o.apply_B(o.propagate(yv))) ** 2 for yv in y_vecs)
+    history = []
+    for n in range(max_iter):
+        total = 0.0
+        for b in range(len(ys)):
+            u = o.propagate(o.apply_B(xs[b]) + y_vecs[b])
+            r = o.apply_B(xs[b] - u)
+            total += np.linalg.norm(r) ** 2
+            xs[b] = xs[b] - ALPHA * r
+        eps = float(np.sqrt(total / nu2))
+        history.append(eps)
+        if eps < tol:
+            break
+    return xs, np.asarray(history)
 
 
 def from_workload(w, n_map=None):

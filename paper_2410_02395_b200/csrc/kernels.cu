@@ -353,12 +353,70 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
     grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, p.finish, RED_RESIDUAL, p.state, p.hist, red);
 }
 
+// Slab pass of the LAST axis (the contiguous one): the t outputs of an item are contiguous voxels.  One thread per
+// output (item, e) with e fastest: the TT threads of an item read the same 2 TT values of d (one 128-byte line, served by
+// L1) and write TT contiguous voxels, instead of one thread writing 64 bytes per row with rows 8 N2 bytes apart.
+template <int TT, bool ACT>
+__global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDesc g, const SlabPassParams p, const unsigned n_items) {
+    __shared__ float Ks[TT * TT];
+    __shared__ double red[32];
+    if (p.state->done) return;
+    constexpr int t = TT;
+    for (int i = threadIdx.x; i < TT * TT; i += SLAB_THREADS) Ks[i] = p.Kh[i];
+    __syncthreads();
+    const unsigned S = (unsigned)g.S[2];
+    const int M = g.M[2];
+    const unsigned n_out = n_items * TT;              // <= voxels < 2^31 (2t <= M)
+    float acc = 0.f;
+    for (unsigned w = blockIdx.x * SLAB_THREADS + threadIdx.x; w < n_out; w += gridDim.x * SLAB_THREADS) {
+        const unsigned item = w / TT;
+        const int e = (int)(w - item * TT);
+        const int side = (int)(item & 1u);
+        const unsigned rest = item >> 1;
+        const unsigned o = rest / S;                  // grid row i0 * N1 + i1
+        const int s = (int)(rest - o * S);
+        if constexpr (ACT) {
+            const int i0 = (int)(o / (unsigned)g.N[1]), i1 = (int)(o - (unsigned)i0 * (unsigned)g.N[1]);
+            if (!p.active[((i0 / g.M[0]) * g.S[1] + i1 / g.M[1]) * g.S[2] + s]) continue;
+        }
+        int nb = side ? s + 1 : s - 1;
+        bool has_nb = true;
+        if (nb < 0 || nb >= (int)S) {
+            if (g.per[2]) nb = (nb + (int)S) % (int)S;
+            else has_nb = false;
+        }
+        // side 1 (last t points of s) reads the FIRST t points of s and s+1; side 0 reads the LAST t points
+        const cf* own = p.ds + ((long long)(o * S + (unsigned)s) * 2 * t + (side ? 0 : t));
+        const cf* nbp = p.ds + ((long long)(o * S + (unsigned)nb) * 2 * t + (side ? 0 : t));
+        float sr = 0.f, si = 0.f;
+#pragma unroll
+        for (int q = 0; q < TT; ++q) {
+            const cf ov = own[q];
+            cf nv = make_float2(0.f, 0.f);
+            if (has_nb) nv = nbp[q];
+            const float k = side ? Ks[e * TT + q] : Ks[q * TT + e];
+            sr = fmaf(k, nv.x - ov.x, sr);
+            si = fmaf(k, nv.y - ov.y, si);
+        }
+        const cf corr = cmul(p.c, make_float2(sr, si));
+        const long long vox = (long long)o * g.N[2] + s * M + (side ? M - t : 0) + e;
+        const cf uu = p.u[vox];
+        const cf r = make_float2(uu.x - corr.x, uu.y - corr.y);
+        const cf xv = p.x[vox];
+        acc += r.x * r.x + r.y * r.y;
+        p.x[vox] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
+    }
+    const double bs = block_sum((double)acc, red);
+    grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, p.finish, RED_RESIDUAL, p.state, p.hist, red);
+}
+
 int slab_pass_blocks(const GridDesc& g, int ax) {
     long long outer = 1, inner = 1;
     for (int d = 0; d < ax; ++d) outer *= g.N[d];
     for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
     const long long n_items = outer * g.S[ax] * 2 * inner;
-    long long nb = (n_items + SLAB_THREADS - 1) / SLAB_THREADS;
+    const long long n_threads = ax == 2 ? n_items * g.t : n_items;    // the last axis runs one thread per output
+    long long nb = (n_threads + SLAB_THREADS - 1) / SLAB_THREADS;
     if (nb > 1024) nb = 1024;
     return (int)(nb < 1 ? 1 : nb);
 }
@@ -373,7 +431,9 @@ cudaError_t launch_slab_pass(const GridDesc& g, const SlabPassParams& p, cudaStr
     const long long n_items = outer * g.S[ax] * 2 * inner;
     const int nb = slab_pass_blocks(g, ax);
 #define MBS_SLAB_PASS(TTv)                                                                                 \
-    if (p.active) k_slab_pass<TTv, true><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items);        \
+    if (ax == 2 && p.active) k_slab_pass_contig<TTv, true><<<nb, SLAB_THREADS, 0, st>>>(g, p, (unsigned)n_items);   \
+    else if (ax == 2) k_slab_pass_contig<TTv, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, (unsigned)n_items);         \
+    else if (p.active) k_slab_pass<TTv, true><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items);   \
     else k_slab_pass<TTv, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items)
     switch (g.t) {
         case 2: MBS_SLAB_PASS(2); break;

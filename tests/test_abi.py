@@ -54,6 +54,9 @@ def test_create_rejects_bad_arguments_without_gpu(lib_path):
         B.mbs_create((176,), 0.25, 1.0, (4,), (2,), None, 8)
     assert e.value.status == B.MBS_ERR_UNSUPPORTED_SIZE
     assert "88" in str(e.value)
+    with pytest.raises(B.MBSError) as e:                      # 2^31 voxels: one more than the kernels' 32-bit counters hold
+        B.mbs_create((2048, 1024, 1024), 0.25, 1.0, (4, 4, 4), (2, 2, 2), None, 8)
+    assert e.value.status == B.MBS_ERR_INVALID_ARG and "2^31" in str(e.value)
 
 
 def test_header_compiles_as_c():

@@ -433,3 +433,34 @@ def test_activation_rule_against_dense_transfer_norm():
             return np.sqrt(sum(np.linalg.norm((C @ xs[n].reshape(-1)).reshape(shape)[blocks[k]]) ** 2 for C in Cd))
         assert T(act[k]) >= thr * nu                        # activated when the transferred norm reaches the threshold
         assert all(T(n) < thr * nu for n in range(act[k]))  # ... and not before
+
+
+# ------------------------------------------------------------------------------------------
+# batched solves (reading R18 in DESIGN.md section 3)
+# ------------------------------------------------------------------------------------------
+def test_batch_is_independent_solves_with_a_stacked_residual():
+    """R18: the sources do not couple (each x_b^(n) is the n-th iterate of its own Eq. (6)), and the one residual
+    of the stacked block-diagonal system is eps_n^2 = sum_b eps_{b,n}^2 nu_b^2 / sum_b nu_b^2 (P:130 applied to it)."""
+    shape, S, t = (16, 12), (2, 1), 4
+    o = _small_oracle(shape, S, (2, 2), t, seed=61)
+    rng = np.random.default_rng(7)
+    ys = [rng.standard_normal(shape) + 1j * rng.standard_normal(shape) for _ in range(3)]
+    ys[1] = np.zeros(shape, dtype=np.complex128)
+    ys[1][3, 4] = 1.0                                   # one sparse source among dense ones
+    n_it = 25
+    xs, hist = orc.solve_batch(o, ys, tol=0.0, max_iter=n_it)
+    singles = [o.solve(y, tol=0.0, max_iter=n_it) for y in ys]
+    L, V = dr.assemble(o.k2, o.k02, o.c, shape, S, t, o.h, o.a, (0, 0))
+    I = np.eye(L.shape[0])
+    nus = [np.linalg.norm((I - V) @ np.linalg.solve(L + I, (-o.c * y).reshape(-1))) for y in ys]   # dense, independent
+    for b in range(3):
+        assert np.linalg.norm(xs[b] - singles[b][0]) <= 1e-13 * np.linalg.norm(singles[b][0])
+    stacked = np.sqrt(sum((singles[b][1] * nus[b]) ** 2 for b in range(3)) / sum(nu ** 2 for nu in nus))
+    assert np.allclose(hist, stacked, rtol=1e-11)
+    assert hist[0] == pytest.approx(1.0, abs=1e-12)     # cold start: eps_0 = 1 for the stacked system too
+    # the stop test acts on the stacked residual: every source gets the same number of updates
+    xs2, hist2 = orc.solve_batch(o, ys, tol=1e-3, max_iter=5000)
+    assert hist2[-1] < 1e-3 and np.all(hist2[:-1] >= 1e-3)
+    for b in range(3):
+        xb, _ = o.solve(ys[b], tol=0.0, max_iter=len(hist2))
+        assert np.linalg.norm(xs2[b] - xb) <= 1e-13 * np.linalg.norm(xb)
