@@ -72,6 +72,8 @@ def parse_args():
     ap.add_argument("--unfused", action="store_true", help="one kernel per step of P:122-128 instead of the fused sweeps")
     ap.add_argument("--opt", action="append", default=[], metavar="NAME=VALUE",
                     help="kernel option for profiling runs, e.g. LINE=2, LINE=0, TMA=0 (enum mbs_option; not the headline)")
+    ap.add_argument("--batch", type=int, default=None, metavar="N",
+                    help="only: time mbs_solve_batch with N sources sharing the medium of --config (P:23; NEXT-4) beside one source")
     ap.add_argument("--activation", type=float, default=None, metavar="THRESHOLD",
                     help="--converge-config only: solve with subdomain activation (P:139-141) at this relative threshold "
                          "(negative: the default tol / 10) and report it beside the plain solve")
@@ -361,6 +363,36 @@ def add_e2e(s, w, y, line, K):
     del yh, xh
 
 
+def batched(cfg, n_batch, K, W, dev):
+    """Throughput of mbs_solve_batch (n_batch sources, one medium) against the same solver with one source: device time of
+    the iteration loop (mbs_info.last_solve_ms; the nu pre-pass is outside it), K updates after W warm-up updates."""
+    import torch
+    from paper_2410_02395_b200 import binding, workloads
+    w = workloads.config(cfg)
+    n_map, y = w.make_medium(), w.make_source()
+    s = binding.Solver.from_workload(w, device=dev)
+    s.set_potential(torch.from_numpy(n_map).to(dev))
+    del n_map
+    peak, peak_kind = peaks()
+    out = {"workload": workload_name(w), "steps": K, "warmup": W, "peak": peak, "runs": []}
+    for nb in (1, n_batch):
+        # the sources: the config's own source shifted along axis 0 (distinct right-hand sides, same sparsity)
+        ys = torch.stack([torch.from_numpy(np.roll(y, 7 * b, axis=0)) for b in range(nb)]).to(dev)
+        xs = torch.zeros_like(ys)
+        binding.mbs_solve_batch(s.ctx, nb, ys.data_ptr(), xs.data_ptr(), -1.0, W, want_history=False)
+        rc, hist, _ = binding.mbs_solve_batch(s.ctx, nb, ys.data_ptr(), xs.data_ptr(), -1.0, K)
+        ms = s.info()["last_solve_ms"]
+        ledger = (96.0 + 16.0 / nb) * w.voxels * nb                 # bytes per iteration of the batch (SURVEY 8(f) NEXT-4)
+        out["runs"].append({"n_batch": nb, "ms_per_iteration": ms / K, "Gvoxel_it_per_s": nb * w.voxels * K / (ms * 1e-3) / 1e9,
+                            "ledger_bytes_per_voxel_iteration_and_source": 96.0 + 16.0 / nb,
+                            "frac_of_own_ledger": ledger * K / (ms * 1e-3) / 1e9 / peak,
+                            "frac_of_112B_roofline": 112.0 * w.voxels * nb * K / (ms * 1e-3) / 1e9 / peak,
+                            "residual_last": float(hist[-1])})
+        del ys, xs
+    s.close()
+    return out
+
+
 def converge(cfg, dev, with_floor=True, activation=None):
     """Seconds to converge (BASELINE.json metric, second part): cold-start mbs_solve of config `cfg` at its tol, and the
     complex64 residual floor of that case (minimum eps when iterating on without a stop test)."""
@@ -419,6 +451,11 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    if args.batch is not None:
+        if rank == 0:
+            cfgb = args.config or 3
+            print(json.dumps({"batched": batched(cfgb, args.batch, args.steps or DEFAULT_STEPS[cfgb], max(args.warmup or 3, 3), dev)}))
+        return
     if args.converge_config is not None:
         if rank == 0:
             out = {"time_to_converge": converge(args.converge_config, dev, with_floor=args.converge_config == 3)}

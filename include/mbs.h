@@ -189,6 +189,23 @@ MBS_API int mbs_solve(mbs_ctx* ctx, const void* y_device, void* x_device, double
               double* residual_history, int32_t* n_iter);
 
 /*
+ * Batched solve: n_batch sources for ONE medium and wavelength (time- or source-dependent problems are solved one
+ * system per source; the systems share A).  Reading R18, the same rule as the oracle's solve_batch:
+ * every source is iterated in lock step with Eq. (6), exactly as mbs_solve would iterate it, and ONE stop test is
+ * applied to the stacked system: eps_n = sqrt(sum_b ||r_b||^2) / sqrt(sum_b ||Gamma^-1 y_vec,b||^2).
+ *  y, x   device, n_batch fields one after the other ([n_batch][shape], complex64); x in/out as in mbs_solve.
+ *  tol    >= 0, or -1 for exactly max_iter updates without a stop test.
+ *  residual_history / n_iter  as in mbs_solve, for the stacked system (every source gets the same number of updates).
+ * What it buys: the first / last sweep read B_diag once per line for the whole batch (112 -> 96 + 16/n_batch bytes per
+ * voxel-iteration and source).  The library allocates n_batch fields of workspace on the first call with a larger batch.
+ * Needs a 2-D or 3-D grid whose contiguous subdomain length has a warp-line sweep (<= 512 voxels), t in {2, 4, 8, 16}, the
+ * default kernel options, no subdomain activation -> MBS_ERR_UNSUPPORTED_SIZE / MBS_ERR_INVALID_ARG otherwise.
+ * n_batch = 1 is mbs_solve.
+ */
+MBS_API int mbs_solve_batch(mbs_ctx* ctx, int32_t n_batch, const void* y_device, void* x_device, double tol, int32_t max_iter,
+                    double* residual_history, int32_t* n_iter);
+
+/*
  * Exactly n_iter updates of Eq. (6) with no stop test: the timed "step" of bench.py.
  *  nu  > 0: the normalisation ||Gamma^-1 y_vec|| to use for residual_history (e.g. mbs_info.norm_rhs
  *           of an earlier solve with the same y); <= 0: computed first as in mbs_solve.

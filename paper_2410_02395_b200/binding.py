@@ -37,7 +37,7 @@ STATUS_NAMES = {0: "MBS_OK", 1: "MBS_ERR_INVALID_ARG", 2: "MBS_ERR_UNSUPPORTED_S
 DECLARED_SYMBOLS = ("mbs_create", "mbs_fft_supported", "mbs_workspace_bytes", "mbs_set_workspace", "mbs_set_option",
                     "mbs_set_potential", "mbs_apply_operator", "mbs_solve", "mbs_solve_host", "mbs_iterate",
                     "mbs_get_info", "mbs_get_kernel_stats", "mbs_reset_kernel_stats", "mbs_destroy", "mbs_last_error",
-                    "mbs_set_activation", "mbs_get_activation", "mbs_apply_B_static")
+                    "mbs_set_activation", "mbs_get_activation", "mbs_apply_B_static", "mbs_solve_batch")
 MBS_STATIC_SCRATCH_BYTES = 16 << 20
 
 
@@ -80,6 +80,8 @@ _lib.mbs_apply_B_static.restype = ctypes.c_int
 _lib.mbs_solve.argtypes = [_vp, _vp, _vp, ctypes.c_double, ctypes.c_int32, ctypes.POINTER(ctypes.c_double),
                            ctypes.POINTER(ctypes.c_int32)]
 _lib.mbs_solve.restype = ctypes.c_int
+_lib.mbs_solve_batch.argtypes = [_vp, ctypes.c_int32] + list(_lib.mbs_solve.argtypes[1:])
+_lib.mbs_solve_batch.restype = ctypes.c_int
 _lib.mbs_solve_host.argtypes = _lib.mbs_solve.argtypes
 _lib.mbs_solve_host.restype = ctypes.c_int
 _lib.mbs_iterate.argtypes = [_vp, _vp, _vp, ctypes.c_int32, ctypes.c_double, ctypes.POINTER(ctypes.c_double)]
@@ -178,6 +180,16 @@ def _solve(fn, ctx, y_ptr, x_ptr, tol, max_iter, want_history):
 def mbs_solve(ctx, y_ptr: int, x_ptr: int, tol: float, max_iter: int, want_history: bool = True):
     """Device pointers.  Returns (status, residual_history, n_iter); status is MBS_OK or MBS_ERR_NOT_CONVERGED."""
     return _solve(_lib.mbs_solve, ctx, y_ptr, x_ptr, tol, max_iter, want_history)
+
+
+def mbs_solve_batch(ctx, n_batch: int, y_ptr: int, x_ptr: int, tol: float, max_iter: int, want_history: bool = True):
+    """n_batch sources, one medium (device pointers to [n_batch][shape] arrays).  Returns (status, history, n_iter)."""
+    hist = np.empty(max_iter if want_history else 0, dtype=np.float64)
+    n_iter = ctypes.c_int32(0)
+    hp = hist.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if want_history else None
+    rc = _lib.mbs_solve_batch(ctx, int(n_batch), _vp(y_ptr), _vp(x_ptr), float(tol), int(max_iter), hp, ctypes.byref(n_iter))
+    _check(ctx, rc, allow=(MBS_ERR_NOT_CONVERGED,))
+    return rc, hist[:n_iter.value], n_iter.value
 
 
 def mbs_solve_host(ctx, y_ptr: int, x_ptr: int, tol: float, max_iter: int, want_history: bool = True):
@@ -308,6 +320,23 @@ class Solver:
                 with torch.cuda.stream(self.stream):
                     xd = xd.clone()
         rc, hist, _ = mbs_solve(self.ctx, yd.data_ptr(), xd.data_ptr(), tol, max_iter)   # returns after a stream sync
+        return xd, hist, rc
+
+    def solve_batch(self, ys, x0s=None, tol: float = 1e-6, max_iter: int = 1000):
+        """ys: [n_batch, *shape] (numpy or tensor).  Returns (x [n_batch, *shape] device tensor, history, status)."""
+        torch = self._torch
+        if not isinstance(ys, torch.Tensor):
+            ys = torch.from_numpy(np.ascontiguousarray(ys))
+        with torch.cuda.stream(self.stream):
+            yd = ys.to(device=self.device, dtype=torch.complex64).contiguous()
+            if x0s is None:
+                xd = torch.zeros_like(yd)
+            else:
+                if not isinstance(x0s, torch.Tensor):
+                    x0s = torch.from_numpy(np.ascontiguousarray(x0s))
+                xd = x0s.to(device=self.device, dtype=torch.complex64).contiguous().clone()
+        assert tuple(yd.shape[1:]) == self.shape and xd.shape == yd.shape
+        rc, hist, _ = mbs_solve_batch(self.ctx, yd.shape[0], yd.data_ptr(), xd.data_ptr(), tol, max_iter)
         return xd, hist, rc
 
     def solve_host(self, y_host, x_host, tol: float, max_iter: int):

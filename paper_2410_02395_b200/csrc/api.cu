@@ -102,6 +102,13 @@ struct mbs_ctx {
     double split_eps = 1.0;          // eps at the last re-centering
     int n_recenter = 0;
 
+    // batched solves (R18): n sources share the medium; their u and compact buffers live here
+    int batch_n = 1;                 // sources of the running mbs_solve_batch (1: plain solve)
+    int batch_cap = 0;
+    cf* batch_u = nullptr;
+    CorrBufs batch_cx{}, batch_ds{};
+    unsigned char* batch_mask = nullptr;
+
     // subdomain activation (R17)
     int activation = 0;
     double act_threshold = -1.0;     // relative to nu; < 0: tol / 10 of the solve
@@ -414,6 +421,17 @@ extern "C" int mbs_create(mbs_ctx** out, int ndim, const int64_t* shape, double 
     return MBS_OK;
 }
 
+static void free_batch(mbs_ctx* c) {
+    if (c->batch_u) cudaFree(c->batch_u);
+    for (int ax = 0; ax < 3; ++ax) {
+        if (c->batch_cx.buf[ax]) cudaFree(c->batch_cx.buf[ax]);
+        if (c->batch_ds.buf[ax]) cudaFree(c->batch_ds.buf[ax]);
+        c->batch_cx.buf[ax] = c->batch_ds.buf[ax] = nullptr;
+    }
+    if (c->batch_mask) cudaFree(c->batch_mask);
+    c->batch_u = nullptr; c->batch_mask = nullptr; c->batch_cap = 0;
+}
+
 extern "C" void mbs_destroy(mbs_ctx* c) {
     if (!c) return;
     if (c->ws_owned && c->ws) cudaFree(c->ws);
@@ -436,6 +454,7 @@ extern "C" void mbs_destroy(mbs_ctx* c) {
     if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
     if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     if (c->act_mem) cudaFree(c->act_mem);
+    free_batch(c);
     if (c->delta) cudaFree(c->delta);
     if (c->dref) cudaFree(c->dref);
     if (c->bdiag64) cudaFree(c->bdiag64);
@@ -651,18 +670,19 @@ static int run_fft_contig(mbs_ctx* c, cf* buf, int mode, int inverse, bool in_lo
 }
 
 // FFT sweep along strided axis ax (0 or 1), in place on buf
-static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, bool in_loop) {
+// n_rep > 1: `buf` holds n_rep fields one after the other (batched solves): the batch is one more outer dimension
+static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, bool in_loop, int n_rep = 1) {
     const GridDesc& g = c->g;
     const FftEntry* e = c->fft[ax];
     StridedGeom sg{};
-    long long inner = 1, outer = 1;
+    long long inner = 1, outer = n_rep;
     for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
     for (int d = 0; d < ax; ++d) outer *= g.N[d];
     sg.stride = inner; sg.outer_stride = (long long)g.N[ax] * inner; sg.n_outer = (int)outer; sg.n_seg = g.S[ax];
     const int cs = (mode == FFT_MID) ? e->CSM : e->CS;
     sg.inner = (int)inner; sg.tiles_inner = (int)((inner + cs - 1) / cs);
     sg.n_tiles = outer * g.S[ax] * sg.tiles_inner;
-    if (in_loop && activation_effective(c) && g.M[2] % cs == 0) {
+    if (in_loop && n_rep == 1 && activation_effective(c) && g.M[2] % cs == 0) {
         // visit only the tiles of the active subdomains (their list lives in device memory)
         sg.act_list = c->act.list; sg.n_act = c->act.n_act; sg.axis = ax;
         sg.tps2 = g.M[2] / cs; sg.tiles_per_sub = (ax == 1 ? g.M[0] : g.M[1]) * sg.tps2;
@@ -678,17 +698,17 @@ static int run_fft_strided(mbs_ctx* c, cf* buf, int ax, int mode, int inverse, b
     }
     static const char* names[2][3] = {{"fft_strided_fwd_ax0", "fft_strided_inv_ax0", "fft_strided_mid_ax0"},
                                       {"fft_strided_fwd_ax1", "fft_strided_inv_ax1", "fft_strided_mid_ax1"}};
-    KernelScope ks(c, names[ax][mode], 16.0 * (double)g.voxels);
+    KernelScope ks(c, names[ax][mode], 16.0 * (double)g.voxels * n_rep);
     MBS_CUDA(c, e->strided(buf, sg, s2, c->tw_dev[ax], mode, in_loop ? &c->state->done : nullptr, c->num_sms, c->use_tma,
                            c->stream));
     return MBS_OK;
 }
 
 // the sweeps between the first and the last one: strided forward, kernel multiply, strided inverse (a3-a5)
-static int run_middle_sweeps(mbs_ctx* c, cf* buf, int inverse, bool in_loop) {
-    if (c->ndim == 3) MBS_TRY(run_fft_strided(c, buf, 1, FFT_FWD, inverse, in_loop));
-    MBS_TRY(run_fft_strided(c, buf, c->first, FFT_MID, inverse, in_loop));
-    if (c->ndim == 3) MBS_TRY(run_fft_strided(c, buf, 1, FFT_INV, inverse, in_loop));
+static int run_middle_sweeps(mbs_ctx* c, cf* buf, int inverse, bool in_loop, int n_rep = 1) {
+    if (c->ndim == 3) MBS_TRY(run_fft_strided(c, buf, 1, FFT_FWD, inverse, in_loop, n_rep));
+    MBS_TRY(run_fft_strided(c, buf, c->first, FFT_MID, inverse, in_loop, n_rep));
+    if (c->ndim == 3) MBS_TRY(run_fft_strided(c, buf, 1, FFT_INV, inverse, in_loop, n_rep));
     return MBS_OK;
 }
 
@@ -840,7 +860,96 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     return MBS_OK;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Batched solves (one system per source, the same A; reading R18 of DESIGN.md section 3).  x and y hold n sources
+// one after the other.  Every source runs Eq. (6) exactly as a plain solve; the warp-line sweeps take the sources
+// of a batch one after the other on the same line, so B_diag is read from DRAM once per line and iteration instead of
+// once per source (112 -> 96 + 16/n bytes per voxel-iteration and source); the strided sweeps see the batch as one more
+// outer dimension; one residual of the stacked system decides the stop.
+// ---------------------------------------------------------------------------------------------
+static bool batch_available(const mbs_ctx* c) {
+    return c->ndim >= 2 && c->fused && fused_available(c) && c->use_line && c->fft[2]->line && slab_pass_supported(c->g.t);
+}
+
+static int ensure_batch(mbs_ctx* c, int n) {
+    if (n <= c->batch_cap) return MBS_OK;
+    free_batch(c);
+    const GridDesc& g = c->g;
+    MBS_CUDA(c, cudaMalloc(&c->batch_u, sizeof(cf) * (size_t)n * (size_t)g.voxels));
+    for (int ax = 0; ax < 3; ++ax) {
+        const size_t ne = corr_elems(g, ax);
+        if (!ne) continue;
+        MBS_CUDA(c, cudaMalloc(&c->batch_cx.buf[ax], sizeof(cf) * ne * n));
+        MBS_CUDA(c, cudaMalloc(&c->batch_ds.buf[ax], sizeof(cf) * ne * n));
+    }
+    MBS_CUDA(c, cudaMalloc(&c->batch_mask, (size_t)n * (size_t)(g.voxels / g.N[2])));
+    c->batch_cap = n;
+    return MBS_OK;
+}
+
+static int run_iteration_batch(mbs_ctx* c, const cf* y, cf* x) {
+    const GridDesc& g = c->g;
+    const FftEntry* e = c->fft[2];
+    const int nb = c->batch_n;
+    const int e0 = g.a[0] > 0, e1 = g.a[1] > 0, e2 = g.a[2] > 0 ? 1 : 0;
+    const int* done = &c->state->done;
+    const double vb = 8.0 * (double)g.voxels;
+    FusedParams p{};
+    p.x = x; p.bdiag = c->bdiag; p.y = y; p.ymask = c->batch_mask; p.ysc = to_cf(-c->c); p.u = c->batch_u;
+    p.N0 = g.N[0]; p.S0 = g.S[0];
+    p.N1 = g.N[1]; p.N2 = g.N[2]; p.S2 = g.S[2]; p.a2 = g.a[2]; p.per2 = g.per[2]; p.t = g.t;
+    p.e0 = e0; p.e1 = e1; p.M0 = g.M[0]; p.M1 = g.M[1]; p.S1 = g.S[1];
+    p.cx0 = c->batch_cx.buf[0]; p.cx1 = c->batch_cx.buf[1];
+    p.ds0 = c->batch_ds.buf[0]; p.ds1 = c->batch_ds.buf[1]; p.ds2 = c->batch_ds.buf[2];
+    p.Kh = c->Kh_dev; p.c = to_cf(c->c); p.alpha = (float)c->alpha;
+    p.n_lines = g.voxels / g.M[2];
+    p.partials = c->partials; p.state = c->state; p.hist = c->hist_dev; p.reduce_mode = RED_RESIDUAL;
+    p.line_variant = c->use_line == 2 ? 1 : 0;
+    p.n_batch = nb; p.batch_stride = g.voxels; p.mask_stride = g.voxels / g.N[2];
+    for (int ax = 0; ax < 3; ++ax) p.cstride[ax] = (long long)corr_elems(g, ax);
+    // corr_0(x), corr_1(x) of every source
+    for (int ax = 0; ax < 2; ++ax) {
+        if (!c->batch_cx.buf[ax]) continue;
+        SlabParams sp{};
+        sp.in = x; sp.out = c->batch_cx.buf[ax]; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
+        sp.state = c->state; sp.check_done = 1;
+        sp.n_batch = nb; sp.in_stride = g.voxels; sp.out_stride = (long long)corr_elems(g, ax);
+        static const char* names[2] = {"slab_ax0", "slab_ax1"};
+        KernelScope ks(c, names[ax], 16.0 * (double)corr_elems(g, ax) * nb);
+        MBS_CUDA(c, launch_slab(g, sp, c->stream));
+    }
+    {
+        KernelScope ks(c, "line_sweep1", (2.0 + c->y_row_fraction) * vb * nb + vb);      // B_diag once per batch
+        MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S1, done, c->num_sms, c->stream));
+    }
+    MBS_TRY(run_middle_sweeps(c, c->batch_u, 1, true, nb));
+    const int nb5 = e->line_blocks(LINE_S5, g.t, p.line_variant, p.n_lines, c->num_sms);
+    if (nb5 < 1) return fail(c, MBS_ERR_CUDA, "line sweep: occupancy query failed");
+    const int mask = (e0 ? 1 : 0) | (e1 ? 2 : 0) | (e2 ? 4 : 0);
+    p.slot0 = 0; p.n_total = nb5; p.finish = mask ? 0 : 1;
+    {
+        KernelScope ks(c, "line_sweep5", 3 * vb * nb + vb);
+        MBS_CUDA(c, e->line(p, c->tw_dev[2], LINE_S5, done, c->num_sms, c->stream));
+    }
+    int slot = nb5;
+    const int last_ax = (mask & 4) ? 2 : ((mask & 2) ? 1 : 0);
+    for (int ax = 0; ax < 3; ++ax) {
+        if (!((mask >> ax) & 1)) continue;
+        SlabPassParams sp{};
+        sp.ds = c->batch_ds.buf[ax]; sp.u = c->batch_u; sp.x = x; sp.Kh = c->Kh_dev; sp.c = to_cf(c->c); sp.axis = ax;
+        sp.e1 = e1; sp.e2 = e2; sp.alpha = (float)c->alpha; sp.partials = c->partials; sp.slot0 = slot;
+        sp.finish = (ax == last_ax) ? 1 : 0; sp.state = c->state; sp.hist = c->hist_dev;
+        sp.n_batch = nb; sp.ds_stride = (long long)corr_elems(g, ax); sp.vox_stride = g.voxels;
+        static const char* names[3] = {"slab_pass_ax0", "slab_pass_ax1", "slab_pass_ax2"};
+        KernelScope ks(c, names[ax], 40.0 * (double)corr_elems(g, ax) * nb);
+        MBS_CUDA(c, launch_slab_pass(g, sp, c->stream));
+        slot += slab_pass_blocks(g, ax);
+    }
+    return MBS_OK;
+}
+
 static int run_iteration(mbs_ctx* c, const cf* y, cf* x) {
+    if (c->batch_n > 1) return run_iteration_batch(c, y, x);
     return (c->fused && fused_available(c)) ? run_iteration_fused(c, y, x) : run_iteration_unfused(c, y, x);
 }
 
@@ -892,7 +1001,7 @@ extern "C" int mbs_apply_operator(mbs_ctx* c, int which, const void* in_device, 
 // ---------------------------------------------------------------------------------------------
 static bool split_effective(const mbs_ctx* c) {
     const bool want = c->refine == 1 || (c->refine < 0 && c->g.voxels <= (1LL << 21));
-    return want && c->fused && fused_available(c) && !c->activation;
+    return want && c->fused && fused_available(c) && !c->activation && c->batch_n == 1;
 }
 
 // double tables and work arrays of refine_f64.cu (once per context)
@@ -974,22 +1083,36 @@ static int recenter(mbs_ctx* c, const cf* y, cf* x, bool add_delta) {
 
 // Reset the device state for a new solve and (nu <= 0) compute nu = || B (L+I)^-1 y_vec ||
 static int begin_solve(mbs_ctx* c, const cf* y, const cf* x, double tol, int32_t max_iter, double nu) {
-    if (c->activation && !activation_effective(c))
-        return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation needs the default kernel options (fused warp-line sweeps)");
+    if (c->activation && (!activation_effective(c) || c->batch_n > 1))
+        return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation needs the default kernel options (fused warp-line sweeps) and a single source");
     DevState init{};
     init.iter = 0; init.done = 0; init.max_iter = max_iter; init.ticket = 0; init.tol = tol;
     init.nu2 = nu > 0 ? nu * nu : 0.0; init.last_sum = 0;
     init.n_active = c->n_sub; init.n_sub = c->n_sub; init.xnorm2 = 0.0;
     c->state_pinned[0] = init;
     MBS_CUDA(c, cudaMemcpyAsync(c->state, &c->state_pinned[0], sizeof(DevState), cudaMemcpyHostToDevice, c->stream));
+    const long long rows = c->g.voxels / c->g.N[2];
     {
-        KernelScope ks(c, "source_row_mask", 8.0 * (double)c->g.voxels);
-        MBS_CUDA(c, launch_row_mask(y, c->ymask, c->g.voxels / c->g.N[2], c->g.N[2], c->stream));
+        KernelScope ks(c, "source_row_mask", 8.0 * (double)c->g.voxels * c->batch_n);
+        MBS_CUDA(c, launch_row_mask(y, c->batch_n > 1 ? c->batch_mask : c->ymask, rows * c->batch_n, c->g.N[2], c->stream));
     }
     if (!(nu > 0)) {
-        { KernelScope ks(c, "scale_copy", 16.0 * (double)c->g.voxels); MBS_CUDA(c, launch_scale_copy(y, c->u, to_cf(-c->c), c->g.voxels, c->stream)); }
-        MBS_TRY(run_propagator(c, c->u, 1, false));
-        MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
+        // nu^2 = sum over the sources of ||B (L+I)^-1 y_vec,b||^2 (one source: the plain normalisation of P:130)
+        double nu2_sum = 0.0;
+        for (int b = 0; b < c->batch_n; ++b) {
+            const cf* yb = y + (size_t)b * (size_t)c->g.voxels;
+            { KernelScope ks(c, "scale_copy", 16.0 * (double)c->g.voxels); MBS_CUDA(c, launch_scale_copy(yb, c->u, to_cf(-c->c), c->g.voxels, c->stream)); }
+            MBS_TRY(run_propagator(c, c->u, 1, false));
+            MBS_TRY(run_B(c, c->u, nullptr, nullptr, make_float2(0.f, 0.f), nullptr, 1.f, nullptr, 0.f, RED_NU2, false));
+            if (c->batch_n > 1) {
+                DevState st{};
+                MBS_CUDA(c, cudaMemcpyAsync(&st, c->state, sizeof(DevState), cudaMemcpyDeviceToHost, c->stream));
+                MBS_CUDA(c, cudaStreamSynchronize(c->stream));
+                nu2_sum += st.nu2;
+            }
+        }
+        if (c->batch_n > 1)
+            MBS_CUDA(c, cudaMemcpy(&c->state->nu2, &nu2_sum, sizeof(double), cudaMemcpyHostToDevice));   // (the stream is idle here)
     }
     if (c->activation) {
         // an inactive subdomain contributes d = 0: the compact d buffers must not hold values of an earlier solve
@@ -1013,9 +1136,9 @@ static int begin_solve(mbs_ctx* c, const cf* y, const cf* x, double tol, int32_t
     MBS_CUDA(c, cudaStreamSynchronize(c->stream));   // state_pinned[0] is reused by the poll loop
     {
         // rows of y the first sweep has to read (byte ledger of the sparse-source row of SURVEY 8(d))
-        const size_t rows = (size_t)(c->g.voxels / c->g.N[2]);
+        const size_t rows = (size_t)(c->g.voxels / c->g.N[2]) * (size_t)c->batch_n;
         std::vector<unsigned char> m(rows);
-        MBS_CUDA(c, cudaMemcpy(m.data(), c->ymask, rows, cudaMemcpyDeviceToHost));
+        MBS_CUDA(c, cudaMemcpy(m.data(), c->batch_n > 1 ? c->batch_mask : c->ymask, rows, cudaMemcpyDeviceToHost));
         size_t nz = 0;
         for (size_t i = 0; i < rows; ++i) nz += m[i] ? 1 : 0;
         c->y_row_fraction = rows ? (double)nz / (double)rows : 1.0;
@@ -1055,7 +1178,7 @@ static int ensure_history(mbs_ctx* c, int32_t max_iter) {
 // Enqueue `batch` iterations: as individual launches, or (graphs on, not profiling) as one replay of a CUDA graph
 // captured from the same launches.  The graph is rebuilt when the arrays, the batch or the kernel options change.
 static bool graphs_enabled(const mbs_ctx* c) {
-    return !c->profile && (c->use_graph == 1 || (c->use_graph < 0 && c->g.voxels <= (1LL << 25)));
+    return !c->profile && c->batch_n == 1 && (c->use_graph == 1 || (c->use_graph < 0 && c->g.voxels <= (1LL << 25)));
 }
 
 static int enqueue_batch(mbs_ctx* c, const cf* y, cf* x, int batch, bool allow_graph) {
@@ -1201,6 +1324,23 @@ extern "C" int mbs_solve(mbs_ctx* c, const void* y_device, void* x_device, doubl
     if (!c) return MBS_ERR_INVALID_ARG;
     if (!(tol >= 0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0");
     return solve_device(c, (const cf*)y_device, (cf*)x_device, tol, max_iter, 0.0, residual_history, n_iter);
+}
+
+extern "C" int mbs_solve_batch(mbs_ctx* c, int32_t n_batch, const void* y_device, void* x_device, double tol, int32_t max_iter,
+                               double* residual_history, int32_t* n_iter) {
+    if (!c) return MBS_ERR_INVALID_ARG;
+    if (n_batch < 1 || n_batch > 64) return fail(c, MBS_ERR_INVALID_ARG, "n_batch must be in [1, 64] (got %d)", n_batch);
+    if (!(tol >= 0) && !(tol == -1.0)) return fail(c, MBS_ERR_INVALID_ARG, "tol must be >= 0 (or -1: exactly max_iter updates, no stop test)");
+    if (n_batch == 1) return solve_device(c, (const cf*)y_device, (cf*)x_device, tol, max_iter, 0.0, residual_history, n_iter);
+    if (!batch_available(c))
+        return fail(c, MBS_ERR_UNSUPPORTED_SIZE, "batched solves need a 2-D or 3-D grid whose contiguous subdomain length has a warp-line sweep "
+                                                 "(up to 512 voxels), t in {2, 4, 8, 16} and the default kernel options");
+    if (c->activation) return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation and batched solves are exclusive");
+    MBS_TRY(ensure_batch(c, n_batch));
+    c->batch_n = n_batch;
+    const int rc = solve_device(c, (const cf*)y_device, (cf*)x_device, tol, max_iter, 0.0, residual_history, n_iter);
+    c->batch_n = 1;
+    return rc;
 }
 
 extern "C" int mbs_iterate(mbs_ctx* c, const void* y_device, void* x_device, int32_t n_iter, double nu,

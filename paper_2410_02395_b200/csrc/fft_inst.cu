@@ -286,8 +286,9 @@ cudaError_t line_launch(const FusedParams& p, const cf* tw, const int* done, int
     bool fast = false;
     cudaError_t e = line_grid<MODE>(p.t, p.line_variant, p.n_lines, num_sms, &nb, &smem, &fast);
     if (e != cudaSuccess) return e;
-    const LineKernel k = line_kernel<MODE>(p.active != nullptr, fast);
-    if (p.active && (e = prepare(k, LINE_WARPS * 32, smem, &bps)) != cudaSuccess) return e;
+    const bool ext = p.active != nullptr || p.n_batch > 1;        // activation and batches run the extended instantiations
+    const LineKernel k = line_kernel<MODE>(ext, fast);
+    if (ext && (e = prepare(k, LINE_WARPS * 32, smem, &bps)) != cudaSuccess) return e;
     k<<<(unsigned)nb, LINE_WARPS * 32, smem, st>>>(p, tw, done);
     return cudaGetLastError();
 }

@@ -240,7 +240,11 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab(const GridDesc g, const S
     if (p.check_done && p.state->done) return;
     for (int i = threadIdx.x; i < TT * TT; i += SLAB_THREADS) Ks[i] = p.Kh[i];
     __syncthreads();
-    slab_items<TT>(g, p, inner, n_items, Ks, blockIdx.x, gridDim.x);
+    SlabParams q = p;
+    for (int b = 0; b < (p.n_batch > 1 ? p.n_batch : 1); ++b) {          // batched solves: one source after the other
+        slab_items<TT>(g, q, inner, n_items, Ks, blockIdx.x, gridDim.x);
+        q.in += p.in_stride; q.out += p.out_stride;
+    }
 }
 
 // Two axes in one launch (the corrections of different axes are independent): blocks [0, nbA) take the items of pA, the
@@ -253,8 +257,12 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pair(const GridDesc g, co
     if (pA.check_done && pA.state->done) return;
     for (int i = threadIdx.x; i < TT * TT; i += SLAB_THREADS) Ks[i] = pA.Kh[i];
     __syncthreads();
-    if (blockIdx.x < nbA) slab_items<TT>(g, pA, innerA, nA, Ks, blockIdx.x, nbA);
-    else slab_items<TT>(g, pB, innerB, nB, Ks, blockIdx.x - nbA, gridDim.x - nbA);
+    SlabParams q = blockIdx.x < nbA ? pA : pB;
+    for (int b = 0; b < (q.n_batch > 1 ? q.n_batch : 1); ++b) {          // batched solves: one source after the other
+        if (blockIdx.x < nbA) slab_items<TT>(g, q, innerA, nA, Ks, blockIdx.x, nbA);
+        else slab_items<TT>(g, q, innerB, nB, Ks, blockIdx.x - nbA, gridDim.x - nbA);
+        q.in += q.in_stride; q.out += q.out_stride;
+    }
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -277,6 +285,11 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
     const int ax = p.axis;
     const int S = g.S[ax], M = g.M[ax];
     float acc = 0.f;
+    const int n_batch = p.n_batch > 1 ? p.n_batch : 1;    // batched solves (R18): one source after the other
+    for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
+    const cf* ds = p.ds + bsrc * p.ds_stride;
+    cf* u = p.u + bsrc * p.vox_stride;
+    cf* x = p.x + bsrc * p.vox_stride;
     for (long long item = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x; item < n_items;
          item += (long long)gridDim.x * SLAB_THREADS) {
         const long long in_i = item % inner;
@@ -305,9 +318,9 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
         cf dv[TT];
 #pragma unroll
         for (int q = 0; q < TT; ++q) {
-            const cf own = p.ds[own0 + q * inner];
+            const cf own = ds[own0 + q * inner];
             cf nbv = make_float2(0.f, 0.f);
-            if (has_nb) nbv = p.ds[nb0 + q * inner];
+            if (has_nb) nbv = ds[nb0 + q * inner];
             dv[q] = make_float2(nbv.x - own.x, nbv.y - own.y);
         }
         // is the voxel an edge point of a later axis?  (constant over the t outputs of this item)
@@ -338,16 +351,17 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
             }
             const cf corr = cmul(p.c, make_float2(sr, si));
             const long long vox = vox0 + e * vstride;
-            const cf uu = p.u[vox];
+            const cf uu = u[vox];
             const cf r = make_float2(uu.x - corr.x, uu.y - corr.y);
             if (later) {
-                p.u[vox] = r;
+                u[vox] = r;
             } else {
-                const cf xv = p.x[vox];
+                const cf xv = x[vox];
                 acc += r.x * r.x + r.y * r.y;
-                p.x[vox] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
+                x[vox] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
             }
         }
+    }
     }
     const double bs = block_sum((double)acc, red);
     grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, p.finish, RED_RESIDUAL, p.state, p.hist, red);
@@ -368,6 +382,11 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDes
     const int M = g.M[2];
     const unsigned n_out = n_items * TT;              // <= voxels < 2^31 (2t <= M)
     float acc = 0.f;
+    const int n_batch = p.n_batch > 1 ? p.n_batch : 1;    // batched solves (R18): one source after the other
+    for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
+    const cf* ds = p.ds + bsrc * p.ds_stride;
+    cf* u = p.u + bsrc * p.vox_stride;
+    cf* x = p.x + bsrc * p.vox_stride;
     for (unsigned w = blockIdx.x * SLAB_THREADS + threadIdx.x; w < n_out; w += gridDim.x * SLAB_THREADS) {
         const unsigned item = w / TT;
         const int e = (int)(w - item * TT);
@@ -386,8 +405,8 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDes
             else has_nb = false;
         }
         // side 1 (last t points of s) reads the FIRST t points of s and s+1; side 0 reads the LAST t points
-        const cf* own = p.ds + ((long long)(o * S + (unsigned)s) * 2 * t + (side ? 0 : t));
-        const cf* nbp = p.ds + ((long long)(o * S + (unsigned)nb) * 2 * t + (side ? 0 : t));
+        const cf* own = ds + ((long long)(o * S + (unsigned)s) * 2 * t + (side ? 0 : t));
+        const cf* nbp = ds + ((long long)(o * S + (unsigned)nb) * 2 * t + (side ? 0 : t));
         float sr = 0.f, si = 0.f;
 #pragma unroll
         for (int q = 0; q < TT; ++q) {
@@ -400,11 +419,12 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDes
         }
         const cf corr = cmul(p.c, make_float2(sr, si));
         const long long vox = (long long)o * g.N[2] + s * M + (side ? M - t : 0) + e;
-        const cf uu = p.u[vox];
+        const cf uu = u[vox];
         const cf r = make_float2(uu.x - corr.x, uu.y - corr.y);
-        const cf xv = p.x[vox];
+        const cf xv = x[vox];
         acc += r.x * r.x + r.y * r.y;
-        p.x[vox] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
+        x[vox] = make_float2(xv.x - p.alpha * r.x, xv.y - p.alpha * r.y);
+    }
     }
     const double bs = block_sum((double)acc, red);
     grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, p.finish, RED_RESIDUAL, p.state, p.hist, red);

@@ -85,29 +85,39 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
         const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
         bool valid = in_range;
         if constexpr (ACT) {
-            valid = valid && p.active[((i0 / p.M0) * p.S1 + i1 / p.M1) * p.S2 + seg] != 0;
-            if (!__any_sync(0xffffffffu, valid)) continue;
+            if (p.active) {
+                valid = valid && p.active[((i0 / p.M0) * p.S1 + i1 / p.M1) * p.S2 + seg] != 0;
+                if (!__any_sync(0xffffffffu, valid)) continue;
+            }
         }
-        long long o0 = -1, o1 = -1;                   // compact row offsets of the axis-0 / axis-1 slabs
+        long long o0b = -1, o1b = -1;                 // compact row offsets of the axis-0 / axis-1 slabs
         if (p.e0) {
             const int q = line_edge_slot(i0, p.M0, TT);
-            if (q >= 0) o0 = ((long long)q * p.N1 + i1) * p.N2 + (long long)seg * M;
+            if (q >= 0) o0b = ((long long)q * p.N1 + i1) * p.N2 + (long long)seg * M;
         }
         if (p.e1) {
             const int q = line_edge_slot(i1, p.M1, TT);
-            if (q >= 0) o1 = ((long long)i0 * (p.S1 * t2) + q) * p.N2 + (long long)seg * M;
+            if (q >= 0) o1b = ((long long)i0 * (p.S1 * t2) + q) * p.N2 + (long long)seg * M;
         }
-        const long long gl = (long long)line * M + jt;    // this lane's first point
-        const long long grow = (long long)row * p.N2;
+        const long long gl0 = (long long)line * M + jt;   // this lane's first point in B_diag (shared by the sources of a batch)
+        // batched solves (R18; the ACT instantiations only): the sources one after the other on the same line
+        const int n_batch = ACT ? (p.n_batch > 1 ? p.n_batch : 1) : 1;
+        for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
+        const long long boff = ACT ? bsrc * p.batch_stride : 0;
+        const long long gl = gl0 + boff;                  // ... and in x, y, u of this source
+        const long long grow = (long long)row * p.N2 + boff;
+        const long long o0 = (ACT && o0b >= 0) ? o0b + bsrc * p.cstride[0] : o0b;
+        const long long o1 = (ACT && o1b >= 0) ? o1b + bsrc * p.cstride[1] : o1b;
+        const long long mrow = (long long)row + (ACT ? bsrc * p.mask_stride : 0);
         cf v[P];
         if constexpr (MODE == LINE_S1) {
             const cf* xb = p.x + gl;
-            const cf* bb = p.bdiag + gl;
+            const cf* bb = p.bdiag + gl0;
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
                 v[m] = cmul(bb[m * T], xb[m * T]);
             });
-            if (p.y != nullptr && (p.ymask == nullptr || p.ymask[row] != 0)) {
+            if (p.y != nullptr && (p.ymask == nullptr || p.ymask[mrow] != 0)) {
                 const cf* yb = p.y + gl;
                 static_for<0, P>([&](auto mc) {
                     constexpr int m = decltype(mc)::value;
@@ -144,7 +154,7 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
                 const unsigned nline = (unit + gridDim.x * NWARP) * LW + lsub;
                 bool want = nline < n_lines;
                 if constexpr (ACT) {
-                    if (want) {
+                    if (want && p.active) {
                         const unsigned nrow = nline / (unsigned)p.S2;
                         const int ni0 = (int)(nrow / (unsigned)p.N1), ni1 = (int)(nrow - (unsigned)ni0 * (unsigned)p.N1);
                         want = p.active[((ni0 / p.M0) * p.S1 + ni1 / p.M1) * p.S2 + (int)(nline - nrow * (unsigned)p.S2)] != 0;
@@ -171,7 +181,7 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
         } else {
             const cf* ub = p.u + gl;
             const cf* xb = p.x + gl;
-            const cf* bb = p.bdiag + gl;
+            const cf* bb = p.bdiag + gl0;
             cf xr[P], br[P];
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
@@ -230,12 +240,13 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
                 }
                 // d at the edge points of the line, for corr_2(d) in the slab pass of the last axis
                 if (first_edge || last_edge) {
-                    cf* d2 = p.ds2 + (long long)row * (p.S2 * t2) + (long long)seg * t2;
+                    cf* d2 = p.ds2 + (long long)row * (p.S2 * t2) + (long long)seg * t2 + (ACT ? bsrc * p.cstride[2] : 0);
                     if (first_edge) d2[jt] = v[0];
                     if (last_edge) d2[TT + k_last] = v[P - 1];
                 }
             }
         }
+        }   // sources of the batch
     }
     if constexpr (MODE == LINE_S5) {
         const double bs = block_sum((double)acc, red);

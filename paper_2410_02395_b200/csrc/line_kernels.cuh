@@ -139,29 +139,40 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
         const int i0 = (int)(row / (unsigned)p.N1), i1 = (int)(row - (unsigned)i0 * (unsigned)p.N1);
         bool act_ok = true;
         if constexpr (ACT) {
-            // the lines of an inactive subdomain are not computed
-            act_ok = in_range && p.active[((i0 / p.M0) * p.S1 + i1 / p.M1) * p.S2 + seg] != 0;
-            if (!__any_sync(0xffffffffu, act_ok)) continue;
+            if (p.active) {
+                // the lines of an inactive subdomain are not computed
+                act_ok = in_range && p.active[((i0 / p.M0) * p.S1 + i1 / p.M1) * p.S2 + seg] != 0;
+                if (!__any_sync(0xffffffffu, act_ok)) continue;
+            }
         }
         const bool valid = in_range && act_ok;
-        long long o0 = -1, o1 = -1;                   // compact row offsets of the axis-0 / axis-1 slabs
+        long long o0b = -1, o1b = -1;                 // compact row offsets of the axis-0 / axis-1 slabs
         if (valid && p.e0) {
             const int q = line_edge_slot(i0, p.M0, t);
-            if (q >= 0) o0 = ((long long)q * p.N1 + i1) * p.N2 + (long long)seg * M;
+            if (q >= 0) o0b = ((long long)q * p.N1 + i1) * p.N2 + (long long)seg * M;
         }
         if (valid && p.e1) {
             const int q = line_edge_slot(i1, p.M1, t);
-            if (q >= 0) o1 = ((long long)i0 * (p.S1 * t2) + q) * p.N2 + (long long)seg * M;
+            if (q >= 0) o1b = ((long long)i0 * (p.S1 * t2) + q) * p.N2 + (long long)seg * M;
         }
-        const long long gl = (long long)line * M;
-        const long long grow = (long long)row * p.N2;
+        const long long gl0 = (long long)line * M;    // offset of the line in B_diag (shared by the sources of a batch)
+        // batched solves (R18; the ACT instantiations only): the sources of a batch one after the other on the same
+        // line, so that B_diag of the line is read from DRAM once (the later reads hit L1 / L2)
+        const int n_batch = ACT ? (p.n_batch > 1 ? p.n_batch : 1) : 1;
+        for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
+        const long long boff = ACT ? bsrc * p.batch_stride : 0;
+        const long long gl = gl0 + boff;              // offset of the line in x, y, u of this source
+        const long long grow = (long long)row * p.N2 + boff;
+        const long long o0 = (ACT && o0b >= 0) ? o0b + bsrc * p.cstride[0] : o0b;
+        const long long o1 = (ACT && o1b >= 0) ? o1b + bsrc * p.cstride[1] : o1b;
+        const long long mrow = (long long)row + (ACT ? bsrc * p.mask_stride : 0);
         cf v[P];
         if constexpr (MODE == LINE_S1) {
-            const bool has_y = valid && p.y != nullptr && (p.ymask == nullptr || p.ymask[row] != 0);
+            const bool has_y = valid && p.y != nullptr && (p.ymask == nullptr || p.ymask[mrow] != 0);
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
                 const int pidx = jt + m * T;
-                v[m] = valid ? cmul(p.bdiag[gl + pidx], p.x[gl + pidx]) : make_float2(0.f, 0.f);
+                v[m] = valid ? cmul(p.bdiag[gl0 + pidx], p.x[gl + pidx]) : make_float2(0.f, 0.f);
             });
             if (has_y) {
                 static_for<0, P>([&](auto mc) {
@@ -195,7 +206,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                 const unsigned nline = (unit + gridDim.x * NWARP) * LW + lsub;
                 bool want = nline < n_lines;
                 if constexpr (ACT) {
-                    if (want) {
+                    if (want && p.active) {
                         const unsigned nrow = nline / (unsigned)p.S2;
                         const int ni0 = (int)(nrow / (unsigned)p.N1), ni1 = (int)(nrow - (unsigned)ni0 * (unsigned)p.N1);
                         want = p.active[((ni0 / p.M0) * p.S1 + ni1 / p.M1) * p.S2 + (int)(nline - nrow * (unsigned)p.S2)] != 0;
@@ -228,7 +239,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
             if constexpr (STAGE_B) {
                 __syncwarp();                                          // the stage is no longer read by the unit before
                 if (valid) {
-                    const cf* src = p.bdiag + gl;
+                    const cf* src = p.bdiag + gl0;
 #pragma unroll
                     for (int i = 0; i < P / 2; ++i) cp_async16(bst + 2 * (jt + i * T), src + 2 * (jt + i * T));
                 }
@@ -238,7 +249,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
             static_for<0, P>([&](auto mc) {
                 constexpr int m = decltype(mc)::value;
                 xr[m] = valid ? p.x[gl + jt + m * T] : make_float2(0.f, 0.f);
-                if constexpr (PREFETCH_B) br[m] = valid ? p.bdiag[gl + jt + m * T] : make_float2(0.f, 0.f);
+                if constexpr (PREFETCH_B) br[m] = valid ? p.bdiag[gl0 + jt + m * T] : make_float2(0.f, 0.f);
             });
             fft_line_forward_warp<PL>(v, scratch, jt, tw);
             if constexpr (STAGE_B) {
@@ -247,7 +258,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
             }
             if (valid) {
                 const bool slab_row = (o0 >= 0) || (o1 >= 0);
-                const long long o2 = (long long)row * (p.S2 * t2) + (long long)seg * t2;
+                const long long o2 = (long long)row * (p.S2 * t2) + (long long)seg * t2 + (ACT ? bsrc * p.cstride[2] : 0);
                 static_for<0, P>([&](auto mc) {
                     constexpr int m = decltype(mc)::value;
                     const int pidx = jt + m * T;
@@ -271,6 +282,7 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                 });
             }
         }
+        }   // sources of the batch
     }
     if constexpr (MODE == LINE_S5) {
         const double bs = block_sum((double)acc, red);

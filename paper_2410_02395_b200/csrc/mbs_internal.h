@@ -82,6 +82,10 @@ struct SlabParams {
     int compact_in;    // 1: `in` is already a compact [outer][S*2t][inner] buffer (fix-up of the fused sweep)
     const DevState* state;
     int check_done;
+    // batched solves (R18): n_batch sources, `in` advances by in_stride and `out` by out_stride elements per source
+    // (0 / 1 source: plain call)
+    int n_batch;
+    long long in_stride, out_stride;
 };
 
 // fix-up of the fused last sweep on the slab rows of axes 0 and 1 (kernels.cu: k_fixup)
@@ -123,6 +127,8 @@ struct SlabPassParams {
     double* hist;
     const int* active; // subdomain activation: flags per subdomain (s0*S1 + s1)*S2 + s2, or nullptr (all active);
                        // the edge voxels of an inactive subdomain are left alone (no update, no residual)
+    int n_batch;       // batched solves: sources (0 / 1: plain); ds advances by ds_stride, u and x by vox_stride per source
+    long long ds_stride, vox_stride;
 };
 int slab_pass_blocks(const GridDesc& g, int ax);
 bool slab_pass_supported(int t);
@@ -182,6 +188,10 @@ struct FusedParams {
     double* hist;
     const int* active;   // subdomain activation: flags per subdomain, or nullptr; lines of an inactive
                          // subdomain are skipped by the warp-line sweeps
+    // batched solves (R18), warp-line sweeps only: n_batch sources share B_diag; x, y, u advance by batch_stride
+    // elements per source, the compact buffers of axis d by cstride[d], ymask by mask_stride rows
+    int n_batch;
+    long long batch_stride, cstride[3], mask_stride;
     int line_variant;    // warp-line sweeps: 0 = the variant with t known at compile time when there is one (t = 8), 1 = generic
     const cf* dref;      // split iterate (api.cu "refinement"): the sweeps run on the small part delta of x = x_ref + delta,
                          // and the last sweep adds d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec) to d = delta - u'; or nullptr

@@ -711,3 +711,64 @@ def test_subdomain_activation_parity(B, orc, name, make, thr):
     import torch
     assert np.array_equal(h2, h_plain) and torch.equal(x2, x_plain)
     s.close()
+
+
+BATCH_CASES = [
+    # shape, S, W, t, periodic, n_batch
+    ((64, 64, 64), (2, 2, 1), (4, 4, 4), 8, None, 3),
+    ((32, 48, 256), (1, 3, 2), (4, 4, 8), 8, None, 2),         # 128-long lines, ragged transverse extents
+    ((128, 256), (2, 1), (8, 8), 8, None, 4),                  # 2-D
+    ((16, 32, 128), (2, 2, 2), (2, 2, 2), 4, (1, 0, 0), 2),    # periodic axis, t = 4
+    ((16, 16, 512), (1, 1, 1), (2, 2, 8), 8, None, 2),         # 512-long lines: one line per warp (compile-time-t last sweep)
+    ((128, 128, 64), (2, 1, 1), (4, 4, 4), 8, None, 2),        # more lines than one wave of warps: several rounds per warp
+]
+
+
+@pytest.mark.parametrize("shape,S,W,t,periodic,nb", BATCH_CASES)
+def test_batched_solve_parity(B, orc, shape, S, W, t, periodic, nb):
+    """mbs_solve_batch (reading R18): n sources for one medium against the oracle's solve_batch on the same seeded
+    inputs: every field <= 1e-5 after a few updates, the stacked residual history, and each source equal to its own
+    plain solve (the sources do not couple)."""
+    import torch
+    s, o, n = make_pair(B, orc, shape, S, W, t, periodic, seed=17)
+    ys = np.stack([workloads.random_field(shape, 40 + b) for b in range(nb)])
+    ys[nb - 1] = 0
+    ys[nb - 1][tuple(d // 3 for d in shape)] = 1.0                       # one point source among dense ones
+    x0s = np.stack([workloads.random_field(shape, 50 + b) for b in range(nb)])
+    n_it = 6
+    x_ref, h_ref = o_batch = orc.solve_batch(o, list(ys), x0s=list(x0s), tol=0.0, max_iter=n_it)
+    xd, hist, rc = s.solve_batch(ys, x0s=x0s, tol=-1.0, max_iter=n_it)
+    assert rc == B.MBS_OK and len(hist) == n_it
+    assert np.allclose(hist, h_ref, rtol=2e-5), (hist, h_ref)
+    for b in range(nb):
+        check_field(xd[b].cpu().numpy(), x_ref[b], OP_TOL, shape, S, t, periodic, what=("batch", b))
+        # the same source on its own (which on these small grids runs the split iterate): the sources do not couple
+        x1, h1, _ = s.solve(ys[b], x0=x0s[b], tol=0.0, max_iter=n_it)
+        assert rel(xd[b].cpu().numpy(), x1.cpu().numpy()) <= OP_TOL
+    s.close()
+
+
+def test_batched_solve_converges_and_refuses_what_it_cannot_do(B, orc):
+    w = workloads.config(3, shape=(64, 64, 64), boundary_width=(8, 8, 8))
+    n = w.make_medium()
+    ys = np.stack([w.make_source(), np.roll(w.make_source(), 5, axis=0)])
+    o = orc.from_workload(w, n)
+    x_ref, h_ref = orc.solve_batch(o, list(ys), tol=w.tol, max_iter=w.max_iter)
+    s = B.Solver.from_workload(w)
+    s.set_potential(n)
+    xd, hist, rc = s.solve_batch(ys, tol=w.tol, max_iter=w.max_iter)
+    assert rc == B.MBS_OK and abs(len(hist) - len(h_ref)) <= 1
+    assert hist[0] == pytest.approx(1.0, abs=1e-5)
+    for b in range(2):
+        check_field(xd[b].cpu().numpy(), x_ref[b], FIELD_TOL, w.shape, w.n_subdomains, w.n_correction, what=("batch solve", b))
+    s.set_activation(True)
+    with pytest.raises(B.MBSError) as e:
+        s.solve_batch(ys, tol=w.tol, max_iter=10)
+    assert e.value.status == B.MBS_ERR_INVALID_ARG
+    s.close()
+    s1 = B.Solver((256,), 0.25, 1.0, (8,), (2,), n_correction=8)         # 1-D: no batched path
+    s1.set_potential(workloads.random_medium((256,), 3))
+    with pytest.raises(B.MBSError) as e:
+        s1.solve_batch(np.zeros((2, 256), dtype=np.complex64), tol=1e-3, max_iter=10)
+    assert e.value.status == B.MBS_ERR_UNSUPPORTED_SIZE
+    s1.close()
