@@ -233,17 +233,23 @@ __device__ __forceinline__ void slab_items(const GridDesc& g, const SlabParams& 
     }
 }
 
-template <int TT>
+// BATCH: batched solves (R18), one source after the other; a separate instantiation so that the plain kernels keep
+// their code exactly (the loop and the parameter copy cost 25-60 % on these latency-bound kernels)
+template <int TT, bool BATCH = false>
 __global__ void __launch_bounds__(SLAB_THREADS) k_slab(const GridDesc g, const SlabParams p, const long long outer,
                                                        const long long inner, const long long n_items) {
     __shared__ float Ks[TT * TT];
     if (p.check_done && p.state->done) return;
     for (int i = threadIdx.x; i < TT * TT; i += SLAB_THREADS) Ks[i] = p.Kh[i];
     __syncthreads();
-    SlabParams q = p;
-    for (int b = 0; b < (p.n_batch > 1 ? p.n_batch : 1); ++b) {          // batched solves: one source after the other
-        slab_items<TT>(g, q, inner, n_items, Ks, blockIdx.x, gridDim.x);
-        q.in += p.in_stride; q.out += p.out_stride;
+    if constexpr (BATCH) {
+        SlabParams q = p;
+        for (int b = 0; b < p.n_batch; ++b) {
+            slab_items<TT>(g, q, inner, n_items, Ks, blockIdx.x, gridDim.x);
+            q.in += p.in_stride; q.out += p.out_stride;
+        }
+    } else {
+        slab_items<TT>(g, p, inner, n_items, Ks, blockIdx.x, gridDim.x);
     }
 }
 
@@ -257,12 +263,8 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pair(const GridDesc g, co
     if (pA.check_done && pA.state->done) return;
     for (int i = threadIdx.x; i < TT * TT; i += SLAB_THREADS) Ks[i] = pA.Kh[i];
     __syncthreads();
-    SlabParams q = blockIdx.x < nbA ? pA : pB;
-    for (int b = 0; b < (q.n_batch > 1 ? q.n_batch : 1); ++b) {          // batched solves: one source after the other
-        if (blockIdx.x < nbA) slab_items<TT>(g, q, innerA, nA, Ks, blockIdx.x, nbA);
-        else slab_items<TT>(g, q, innerB, nB, Ks, blockIdx.x - nbA, gridDim.x - nbA);
-        q.in += q.in_stride; q.out += q.out_stride;
-    }
+    if (blockIdx.x < nbA) slab_items<TT>(g, pA, innerA, nA, Ks, blockIdx.x, nbA);
+    else slab_items<TT>(g, pB, innerB, nB, Ks, blockIdx.x - nbA, gridDim.x - nbA);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -273,7 +275,7 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pair(const GridDesc g, co
 // its last correction:  |r|^2 partial sum,  x <- x - alpha r        (a7-a9).
 // Passes run in axis order 0, 1, 2 on the stream; the last one finishes the reduction and the stop test.
 // ---------------------------------------------------------------------------------------------
-template <int TT, bool ACT>
+template <int TT, bool ACT, bool BATCH>
 __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, const SlabPassParams p, const long long outer,
                                                             const long long inner, const long long n_items) {
     __shared__ float Ks[TT * TT];
@@ -285,11 +287,11 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
     const int ax = p.axis;
     const int S = g.S[ax], M = g.M[ax];
     float acc = 0.f;
-    const int n_batch = p.n_batch > 1 ? p.n_batch : 1;    // batched solves (R18): one source after the other
+    const int n_batch = BATCH ? p.n_batch : 1;            // batched solves (R18): one source after the other
     for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
-    const cf* ds = p.ds + bsrc * p.ds_stride;
-    cf* u = p.u + bsrc * p.vox_stride;
-    cf* x = p.x + bsrc * p.vox_stride;
+    const cf* __restrict__ ds = BATCH ? p.ds + bsrc * p.ds_stride : p.ds;
+    cf* u = BATCH ? p.u + bsrc * p.vox_stride : p.u;
+    cf* x = BATCH ? p.x + bsrc * p.vox_stride : p.x;
     for (long long item = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x; item < n_items;
          item += (long long)gridDim.x * SLAB_THREADS) {
         const long long in_i = item % inner;
@@ -370,7 +372,7 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
 // Slab pass of the LAST axis (the contiguous one): the t outputs of an item are contiguous voxels.  One thread per
 // output (item, e) with e fastest: the TT threads of an item read the same 2 TT values of d (one 128-byte line, served by
 // L1) and write TT contiguous voxels, instead of one thread writing 64 bytes per row with rows 8 N2 bytes apart.
-template <int TT, bool ACT>
+template <int TT, bool ACT, bool BATCH>
 __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDesc g, const SlabPassParams p, const unsigned n_items) {
     __shared__ float Ks[TT * TT];
     __shared__ double red[32];
@@ -382,11 +384,11 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDes
     const int M = g.M[2];
     const unsigned n_out = n_items * TT;              // <= voxels < 2^31 (2t <= M)
     float acc = 0.f;
-    const int n_batch = p.n_batch > 1 ? p.n_batch : 1;    // batched solves (R18): one source after the other
+    const int n_batch = BATCH ? p.n_batch : 1;            // batched solves (R18): one source after the other
     for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
-    const cf* ds = p.ds + bsrc * p.ds_stride;
-    cf* u = p.u + bsrc * p.vox_stride;
-    cf* x = p.x + bsrc * p.vox_stride;
+    const cf* __restrict__ ds = BATCH ? p.ds + bsrc * p.ds_stride : p.ds;
+    cf* u = BATCH ? p.u + bsrc * p.vox_stride : p.u;
+    cf* x = BATCH ? p.x + bsrc * p.vox_stride : p.x;
     for (unsigned w = blockIdx.x * SLAB_THREADS + threadIdx.x; w < n_out; w += gridDim.x * SLAB_THREADS) {
         const unsigned item = w / TT;
         const int e = (int)(w - item * TT);
@@ -430,12 +432,18 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDes
     grid_reduce_finish(bs, p.partials, p.slot0, p.slot0 + (int)gridDim.x, p.finish, RED_RESIDUAL, p.state, p.hist, red);
 }
 
+// The pass of the contiguous axis runs one thread per output (k_slab_pass_contig) while it is latency-bound: measured 6 %
+// faster at config 3 (131 072 items) and 5-12 % slower at configs 4 and 5 (1.6 M and 4.2 M items) than one thread per item.
+static bool slab_pass_contig(const GridDesc& g, int ax) {
+    return ax == 2 && (long long)g.N[0] * g.N[1] * g.S[2] * 2 <= (1LL << 18);
+}
+
 int slab_pass_blocks(const GridDesc& g, int ax) {
     long long outer = 1, inner = 1;
     for (int d = 0; d < ax; ++d) outer *= g.N[d];
     for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
     const long long n_items = outer * g.S[ax] * 2 * inner;
-    const long long n_threads = ax == 2 ? n_items * g.t : n_items;    // the last axis runs one thread per output
+    const long long n_threads = slab_pass_contig(g, ax) ? n_items * g.t : n_items;    // one thread per output there
     long long nb = (n_threads + SLAB_THREADS - 1) / SLAB_THREADS;
     if (nb > 1024) nb = 1024;
     return (int)(nb < 1 ? 1 : nb);
@@ -450,11 +458,14 @@ cudaError_t launch_slab_pass(const GridDesc& g, const SlabPassParams& p, cudaStr
     for (int d = ax + 1; d < 3; ++d) inner *= g.N[d];
     const long long n_items = outer * g.S[ax] * 2 * inner;
     const int nb = slab_pass_blocks(g, ax);
-#define MBS_SLAB_PASS(TTv)                                                                                 \
-    if (ax == 2 && p.active) k_slab_pass_contig<TTv, true><<<nb, SLAB_THREADS, 0, st>>>(g, p, (unsigned)n_items);   \
-    else if (ax == 2) k_slab_pass_contig<TTv, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, (unsigned)n_items);         \
-    else if (p.active) k_slab_pass<TTv, true><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items);   \
-    else k_slab_pass<TTv, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items)
+#define MBS_SLAB_PASS(TTv)                                                                                                  \
+    if (contig && p.n_batch > 1) k_slab_pass_contig<TTv, false, true><<<nb, SLAB_THREADS, 0, st>>>(g, p, (unsigned)n_items);      \
+    else if (contig && p.active) k_slab_pass_contig<TTv, true, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, (unsigned)n_items);      \
+    else if (contig) k_slab_pass_contig<TTv, false, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, (unsigned)n_items);                 \
+    else if (p.n_batch > 1) k_slab_pass<TTv, false, true><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items);              \
+    else if (p.active) k_slab_pass<TTv, true, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items);                   \
+    else k_slab_pass<TTv, false, false><<<nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items)
+    const bool contig = slab_pass_contig(g, ax);
     switch (g.t) {
         case 2: MBS_SLAB_PASS(2); break;
         case 4: MBS_SLAB_PASS(4); break;
@@ -527,10 +538,14 @@ cudaError_t launch_slab(const GridDesc& g, const SlabParams& p, cudaStream_t st)
     if (nb > 65535LL * 16) nb = 65535LL * 16;
     if (nb < 1) nb = 1;
     switch (g.t) {
-        case 2: k_slab<2><<<(unsigned)nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
-        case 4: k_slab<4><<<(unsigned)nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
-        case 8: k_slab<8><<<(unsigned)nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
-        case 16: k_slab<16><<<(unsigned)nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items); break;
+#define MBS_SLAB(TTv)                                                                                          \
+    if (p.n_batch > 1) k_slab<TTv, true><<<(unsigned)nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items);     \
+    else k_slab<TTv, false><<<(unsigned)nb, SLAB_THREADS, 0, st>>>(g, p, outer, inner, n_items)
+        case 2: MBS_SLAB(2); break;
+        case 4: MBS_SLAB(4); break;
+        case 8: MBS_SLAB(8); break;
+        case 16: MBS_SLAB(16); break;
+#undef MBS_SLAB
         default: {
             long long nb2 = (n_items * g.t + SLAB_THREADS - 1) / SLAB_THREADS;
             if (nb2 > 65535LL * 16) nb2 = 65535LL * 16;
