@@ -93,7 +93,7 @@ struct mbs_ctx {
     // split iterate x = x_ref + delta (lifts the complex64 residual floor on small grids; see recenter())
     int refine = -1;                 // MBS_OPT_REFINE: -1 automatic (grids of <= 2^21 voxels), 0 off, 1 on
     cf* delta = nullptr;             // owned: the small part of the iterate
-    cf* dref = nullptr;              // owned: d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec)
+    cf* dref = nullptr;              // owned: r_ref = B d_ref (complex128 path) or d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec)
     double* bdiag64 = nullptr;       // owned: B_diag in complex128 (grids that may use the split iterate)
     double* Kh64_dev = nullptr;      // owned: K_t / h^2 in double
     double* tw64_dev[3] = {nullptr, nullptr, nullptr};   // owned: double twiddle tables per axis
@@ -770,7 +770,8 @@ static int run_iteration_fused(mbs_ctx* c, const cf* y, cf* x) {
     p.n_lines = g.voxels / g.M[2];
     p.n_tiles = (p.n_lines + e->CC - 1) / e->CC;
     p.partials = c->partials; p.state = c->state; p.hist = c->hist_dev; p.reduce_mode = RED_RESIDUAL;
-    p.dref = c->split ? c->dref : nullptr;
+    p.dref = (c->split && !c->bdiag64) ? c->dref : nullptr;
+    p.rref = (c->split && c->bdiag64) ? c->dref : nullptr;
     p.line_variant = c->use_line == 2 ? 1 : 0;
     const double vb = 8.0 * (double)g.voxels;
     if (c->ndim == 1) {
@@ -1047,9 +1048,9 @@ static int recenter(mbs_ctx* c, const cf* y, cf* x, bool add_delta) {
         r.c_re = c->c.real(); r.c_im = c->c.imag(); r.k02_re = c->k02.real(); r.k02_im = c->k02.imag(); r.h = c->h;
         r.first_axis = c->first;
         {
-            KernelScope ks(c, "recenter_dref_f64", 3 * vb);
-            c->launches += 2 * c->ndim + 2;                   // (the scope counted one of the 2 ndim + 3 launches)
-            MBS_CUDA(c, launch_dref_f64(c->g, r, x, y, c->dref, c->stream));
+            KernelScope ks(c, "recenter_rref_f64", 3 * vb);
+            c->launches += 2 * c->ndim + 4;                   // (the scope counted one of the 2 ndim + 5 launches)
+            MBS_CUDA(c, launch_rref_f64(c->g, r, x, y, c->dref, c->stream));
         }
         MBS_CUDA(c, cudaMemsetAsync(c->delta, 0, bytes, c->stream));
         c->n_recenter++;

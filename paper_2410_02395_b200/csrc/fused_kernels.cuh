@@ -147,6 +147,11 @@ __device__ __forceinline__ float fused_epi_line(const FusedParams& p, const cf* 
                 if (q + 1 < t) r1 = csub(r1, cel[q + 1]);
                 else if (q + 1 >= M - t) r1 = csub(r1, cel[q + 1 - (M - 2 * t)]);
             }
+            if (p.rref) {                                     // split iterate, complex128 residual: r = r_ref + B (delta - u')
+                const cf2 rv = ld2(p.rref + gl + q);
+                r0 = cadd(r0, rv.a);
+                r1 = cadd(r1, rv.b);
+            }
             if constexpr (!SLAB) {
                 acc += r0.x * r0.x + r0.y * r0.y + r1.x * r1.x + r1.y * r1.y;
                 st2(xout + q, make_float2(xv.a.x - p.alpha * r0.x, xv.a.y - p.alpha * r0.y),

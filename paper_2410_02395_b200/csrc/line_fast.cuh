@@ -212,7 +212,9 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
                     // a row in a slab of axis 0 / 1: d to the compact buffers, r_part in place in u; the slab passes finish it
                     static_for<0, P>([&](auto mc) {
                         constexpr int m = decltype(mc)::value;
-                        uo[m * T] = cmul(br[m], v[m]);
+                        cf r = cmul(br[m], v[m]);
+                        if (p.rref) r = cadd(r, p.rref[gl + m * T]);   // split iterate, complex128 residual
+                        uo[m * T] = r;
                     });
                     if (o0 >= 0) {
                         cf* db = p.ds0 + o0 + jt;
@@ -226,7 +228,8 @@ __device__ __forceinline__ void line_body_fast(const FusedParams& p, const cf* _
                     // every point that is not one of the 2 TT edge points of the line is finished here (a7-a9)
                     static_for<0, P>([&](auto mc) {
                         constexpr int m = decltype(mc)::value;
-                        const cf r = cmul(br[m], v[m]);
+                        cf r = cmul(br[m], v[m]);
+                        if (p.rref) r = cadd(r, p.rref[gl + m * T]);   // split iterate, complex128 residual
                         bool edge = false;
                         if constexpr (m == 0) edge = first_edge;
                         if constexpr (m == P - 1) edge = edge || last_edge;

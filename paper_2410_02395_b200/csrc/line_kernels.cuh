@@ -268,7 +268,8 @@ __device__ __forceinline__ void line_body(const FusedParams& p, const cf* __rest
                     cf bv;
                     if constexpr (PREFETCH_B) bv = br[m];
                     else bv = bst[pidx];
-                    const cf r = cmul(bv, d);
+                    cf r = cmul(bv, d);
+                    if (p.rref) r = cadd(r, p.rref[gl + pidx]);        // split iterate, complex128 residual: r = r_ref + B (delta - u')
                     const bool edge2 = p.a2 && (pidx < t || pidx >= M - t);
                     if (!slab_row && !edge2) {
                         acc += r.x * r.x + r.y * r.y;

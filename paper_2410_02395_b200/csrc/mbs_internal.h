@@ -193,6 +193,8 @@ struct FusedParams {
     int n_batch;
     long long batch_stride, cstride[3], mask_stride;
     int line_variant;    // warp-line sweeps: 0 = the variant with t known at compile time when there is one (t = 8), 1 = generic
+    const cf* rref;      // split iterate with the complex128 residual: r_ref = B d_ref, added to r = B_diag d - corr(d) of the
+                         // small part d = delta - u' (instead of d_ref being added to d); or nullptr
     const cf* dref;      // split iterate (api.cu "refinement"): the sweeps run on the small part delta of x = x_ref + delta,
                          // and the last sweep adds d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec) to d = delta - u'; or nullptr
 };
@@ -228,8 +230,8 @@ struct RefineF64 {
     double c_re, c_im, k02_re, k02_im, h;
     int first_axis;        // first real axis of the internal 3-D description
 };
-// dref = x - (L+I)^-1 (B x + y_vec) evaluated in complex128, rounded once to complex64 (y may be nullptr)
-cudaError_t launch_dref_f64(const GridDesc& g, const RefineF64& r, const cf* x, const cf* y, cf* dref, cudaStream_t st);
+// rref = B (x - (L+I)^-1 (B x + y_vec)) evaluated in complex128, rounded once to complex64 (y may be nullptr)
+cudaError_t launch_rref_f64(const GridDesc& g, const RefineF64& r, const cf* x, const cf* y, cf* rref, cudaStream_t st);
 
 // FFT registry (fft_inst.cu compiled once per size, fft_registry.cu)
 struct FftEntry {

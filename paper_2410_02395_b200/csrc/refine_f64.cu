@@ -1,4 +1,4 @@
-// refine_f64.cu -- double-precision evaluation of  d_ref = x_ref - (L+I)^-1 (B x_ref + y_vec)  for the split iterate
+// refine_f64.cu -- double-precision evaluation of  r_ref = B (x_ref - (L+I)^-1 (B x_ref + y_vec))  for the split iterate
 // (api.cu recenter(); DESIGN.md section 6 "Split iterate").
 //
 // Mixed-precision iterative refinement: the iteration of Eq. (6) runs in complex64 on the small part delta of
@@ -9,7 +9,9 @@
 //   k_bxy     u = B_diag x + ysc y - sum_d corr_d(x)         (Eq. (8); corrections evaluated per edge voxel)
 //   k_dft     naive O(M) sum per output along one axis of a subdomain, twiddles from a double table
 //   k_symbol  multiply by 1 / (c (k0^2 - |p|^2) + 1) / prod M_d
-//   k_dref    d_ref = x_ref - u, rounded once to complex64
+//   k_dref    d_ref = x_ref - u;  then k_bxy again: r_ref = B d_ref;  k_round: rounded once to complex64
+// The complex64 last sweep then forms r = r_ref + B_diag (delta - u') - corr(delta - u'): its rounding (B_diag in complex64
+// included) touches only the small part.
 #include "mbs_internal.h"
 
 namespace mbs {
@@ -19,11 +21,13 @@ __device__ __forceinline__ cd2 zmul(cd2 a, cd2 b) { return make_double2(a.x * b.
 __device__ __forceinline__ cd2 zadd(cd2 a, cd2 b) { return make_double2(a.x + b.x, a.y + b.y); }
 __device__ __forceinline__ cd2 zsub(cd2 a, cd2 b) { return make_double2(a.x - b.x, a.y - b.y); }
 __device__ __forceinline__ cd2 to_z(cf a) { return make_double2((double)a.x, (double)a.y); }
+__device__ __forceinline__ cd2 to_z(cd2 a) { return a; }
 
 // corr_ax(x) at the voxel with index i along axis `ax` (other indices fixed through base / stride), or 0 if it is no edge point
 //   first t points of s (b = e):          c sum_a K[a][b] (x_{s-1}[M-t+a] - x_s[M-t+a])
 //   last  t points of s (a = e - (M-t)):  c sum_b K[a][b] (x_{s+1}[b]     - x_s[b])         (P:124-128 read with P:106)
-__device__ __forceinline__ cd2 corr_at(const GridDesc& g, const cf* __restrict__ x, const double* __restrict__ K, const cd2 c,
+template <class T>
+__device__ __forceinline__ cd2 corr_at(const GridDesc& g, const T* __restrict__ x, const double* __restrict__ K, const cd2 c,
                                        const int ax, const int i, const long long base, const long long stride) {
     cd2 out = make_double2(0.0, 0.0);
     if (g.a[ax] == 0 || g.t == 0) return out;
@@ -45,12 +49,12 @@ __device__ __forceinline__ cd2 corr_at(const GridDesc& g, const cf* __restrict__
         double sr = 0.0, si = 0.0;
         for (int q = 0; q < t; ++q) {
             const double kk = is_last ? K[k * t + q] : K[q * t + k];
-            const cf ov = x[base + (long long)(s * M + off + q) * stride];
-            double dx = -(double)ov.x, dy = -(double)ov.y;
+            const cd2 ov = to_z(x[base + (long long)(s * M + off + q) * stride]);
+            double dx = -ov.x, dy = -ov.y;
             if (has_nb) {
-                const cf nv = x[base + (long long)(nb * M + off + q) * stride];
-                dx += (double)nv.x;
-                dy += (double)nv.y;
+                const cd2 nv = to_z(x[base + (long long)(nb * M + off + q) * stride]);
+                dx += nv.x;
+                dy += nv.y;
             }
             sr += kk * dx;
             si += kk * dy;
@@ -60,7 +64,8 @@ __device__ __forceinline__ cd2 corr_at(const GridDesc& g, const cf* __restrict__
     return out;
 }
 
-__global__ void __launch_bounds__(256) k_bxy_f64(const GridDesc g, const cf* __restrict__ x, const cf* __restrict__ y, const cd2 ysc,
+template <class T>
+__global__ void __launch_bounds__(256) k_bxy_f64(const GridDesc g, const T* __restrict__ x, const cf* __restrict__ y, const cd2 ysc,
                                                  const cd2* __restrict__ bdiag, const double* __restrict__ K, const cd2 c,
                                                  cd2* __restrict__ out) {
     const long long s1 = g.N[2], s0 = (long long)g.N[1] * g.N[2];
@@ -130,10 +135,17 @@ __global__ void __launch_bounds__(256) k_symbol_f64(const GridDesc g, cd2* __res
     }
 }
 
+// d = x - u in complex128
 __global__ void __launch_bounds__(256) k_dref_f64(const long long n, const cf* __restrict__ x, const cd2* __restrict__ u,
-                                                  cf* __restrict__ dref) {
+                                                  cd2* __restrict__ d) {
     for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (long long)gridDim.x * blockDim.x)
-        dref[idx] = make_float2((float)((double)x[idx].x - u[idx].x), (float)((double)x[idx].y - u[idx].y));
+        d[idx] = make_double2((double)x[idx].x - u[idx].x, (double)x[idx].y - u[idx].y);
+}
+
+// complex128 -> complex64, rounded once
+__global__ void __launch_bounds__(256) k_round_f64(const long long n, const cd2* __restrict__ in, cf* __restrict__ out) {
+    for (long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x; idx < n; idx += (long long)gridDim.x * blockDim.x)
+        out[idx] = make_float2((float)in[idx].x, (float)in[idx].y);
 }
 
 static unsigned grid_for(long long n) {
@@ -142,10 +154,11 @@ static unsigned grid_for(long long n) {
     return (unsigned)(nb < 1 ? 1 : nb);
 }
 
-cudaError_t launch_dref_f64(const GridDesc& g, const RefineF64& r, const cf* x, const cf* y, cf* dref, cudaStream_t st) {
+// r_ref = B (x - (L+I)^-1 (B x + y_vec)), every step in complex128, rounded once to complex64 at the end (y may be nullptr)
+cudaError_t launch_rref_f64(const GridDesc& g, const RefineF64& r, const cf* x, const cf* y, cf* rref, cudaStream_t st) {
     const unsigned nb = grid_for(g.voxels);
     const cd2 c = make_double2(r.c_re, r.c_im), ysc = make_double2(-r.c_re, -r.c_im);          // y_vec = -c y
-    k_bxy_f64<<<nb, 256, 0, st>>>(g, x, y, ysc, (const cd2*)r.bdiag, r.Kh, c, (cd2*)r.buf[0]);
+    k_bxy_f64<cf><<<nb, 256, 0, st>>>(g, x, y, ysc, (const cd2*)r.bdiag, r.Kh, c, (cd2*)r.buf[0]);
     int cur = 0;
     for (int ax = 2; ax >= r.first_axis; --ax) {                                               // forward transforms
         k_dft_f64<<<nb, 256, 0, st>>>(g, (const cd2*)r.buf[cur], (cd2*)r.buf[cur ^ 1], (const cd2*)r.tw[ax], ax, 0);
@@ -159,7 +172,9 @@ cudaError_t launch_dref_f64(const GridDesc& g, const RefineF64& r, const cf* x, 
         k_dft_f64<<<nb, 256, 0, st>>>(g, (const cd2*)r.buf[cur], (cd2*)r.buf[cur ^ 1], (const cd2*)r.tw[ax], ax, 1);
         cur ^= 1;
     }
-    k_dref_f64<<<nb, 256, 0, st>>>(g.voxels, x, (const cd2*)r.buf[cur], dref);
+    k_dref_f64<<<nb, 256, 0, st>>>(g.voxels, x, (const cd2*)r.buf[cur], (cd2*)r.buf[cur ^ 1]);      // d_ref = x - u
+    k_bxy_f64<cd2><<<nb, 256, 0, st>>>(g, (const cd2*)r.buf[cur ^ 1], nullptr, ysc, (const cd2*)r.bdiag, r.Kh, c, (cd2*)r.buf[cur]);   // B d_ref
+    k_round_f64<<<nb, 256, 0, st>>>(g.voxels, (const cd2*)r.buf[cur], rref);
     return cudaGetLastError();
 }
 
