@@ -458,7 +458,9 @@ def main():
         return
     if args.converge_config is not None:
         if rank == 0:
-            out = {"time_to_converge": converge(args.converge_config, dev, with_floor=args.converge_config == 3)}
+            out = {}
+            if not (args.no_converge and args.activation is not None):      # --no-converge + --activation: the activated solve only
+                out["time_to_converge"] = converge(args.converge_config, dev, with_floor=args.converge_config == 3)
             if args.activation is not None:
                 out["time_to_converge_with_activation"] = converge(args.converge_config, dev, with_floor=False,
                                                                    activation=args.activation)
