@@ -25,7 +25,8 @@ Readings of points the paper leaves open (listed in DESIGN.md section 3, after S
 
 Pins (tests/test_oracle_pins.py, `-m "not gpu"`): printed K_t / sigma_max values, Eq. (9) -> Eq. (4),
 dense assembly from explicit DFT matrices, dense direct solve, monotone residual, eps_0 = 1,
-closed-form 1D Green's function, full-correction identity, corner identity of P:106.
+closed-form 1D Green's function (n = 1 and n = 1.33), full-correction identity, corner identity of P:106, literal values of c,
+alpha through the first two updates, the 2-D absorber corner, the activation rule (R17) and the stacked batch residual (R18).
 The converged fields of the five synthetic BASELINE.json media have no value printed in the paper:
 for them "parity unpinned" beyond those invariants (last row).
 """
