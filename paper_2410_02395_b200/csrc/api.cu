@@ -111,6 +111,7 @@ struct mbs_ctx {
 
     // subdomain activation (R17)
     int activation = 0;
+    bool act_all = false;            // every subdomain of the running solve is active: back to the plain kernels
     double act_threshold = -1.0;     // relative to nu; < 0: tol / 10 of the solve
     ActivationState act{};
     void* act_mem = nullptr;
@@ -511,7 +512,7 @@ extern "C" int mbs_set_option(mbs_ctx* c, int option, int64_t value) {
 // ---------------------------------------------------------------------------------------------
 static bool fused_available(const mbs_ctx* c);
 static bool activation_effective(const mbs_ctx* c) {
-    return c->activation && c->ndim >= 2 && c->fused && fused_available(c) && c->use_line && c->fft[2]->line &&
+    return c->activation && !c->act_all && c->ndim >= 2 && c->fused && fused_available(c) && c->use_line && c->fft[2]->line &&
            slab_pass_supported(c->g.t);
 }
 
@@ -1084,6 +1085,7 @@ static int recenter(mbs_ctx* c, const cf* y, cf* x, bool add_delta) {
 
 // Reset the device state for a new solve and (nu <= 0) compute nu = || B (L+I)^-1 y_vec ||
 static int begin_solve(mbs_ctx* c, const cf* y, const cf* x, double tol, int32_t max_iter, double nu) {
+    c->act_all = false;
     if (c->activation && (!activation_effective(c) || c->batch_n > 1))
         return fail(c, MBS_ERR_INVALID_ARG, "subdomain activation needs the default kernel options (fused warp-line sweeps) and a single source");
     DevState init{};
@@ -1261,6 +1263,11 @@ static int solve_device(mbs_ctx* c, const cf* y, cf* x, double tol, int32_t max_
             pending[prev] = false;
             const DevState& st = c->state_pinned[prev];
             if (st.done) { final_done = st.done; break; }
+            if (c->activation && !c->act_all && st.n_active == st.n_sub) {
+                // every subdomain is awake: the rest of the solve runs the plain kernels (no flags, no activation step)
+                c->act_all = true;
+                invalidate_graph(c);
+            }
             if (c->split && st.iter > 0 && st.nu2 > 0 && c->n_recenter < 64) {
                 // split iterate: re-centre as the residual falls (what is enqueued here runs after the batch already in
                 // flight; in exact arithmetic it changes nothing).  With the double-precision residual (bdiag64) every
