@@ -290,8 +290,8 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass(const GridDesc g, co
     const int n_batch = BATCH ? p.n_batch : 1;            // batched solves (R18): one source after the other
     for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
     const cf* __restrict__ ds = BATCH ? p.ds + bsrc * p.ds_stride : p.ds;
-    cf* u = BATCH ? p.u + bsrc * p.vox_stride : p.u;
-    cf* x = BATCH ? p.x + bsrc * p.vox_stride : p.x;
+    cf* __restrict__ u = BATCH ? p.u + bsrc * p.vox_stride : p.u;      // u, x and ds are distinct arrays
+    cf* __restrict__ x = BATCH ? p.x + bsrc * p.vox_stride : p.x;
     for (long long item = (long long)blockIdx.x * SLAB_THREADS + threadIdx.x; item < n_items;
          item += (long long)gridDim.x * SLAB_THREADS) {
         const long long in_i = item % inner;
@@ -387,8 +387,8 @@ __global__ void __launch_bounds__(SLAB_THREADS) k_slab_pass_contig(const GridDes
     const int n_batch = BATCH ? p.n_batch : 1;            // batched solves (R18): one source after the other
     for (int bsrc = 0; bsrc < n_batch; ++bsrc) {
     const cf* __restrict__ ds = BATCH ? p.ds + bsrc * p.ds_stride : p.ds;
-    cf* u = BATCH ? p.u + bsrc * p.vox_stride : p.u;
-    cf* x = BATCH ? p.x + bsrc * p.vox_stride : p.x;
+    cf* __restrict__ u = BATCH ? p.u + bsrc * p.vox_stride : p.u;      // u, x and ds are distinct arrays
+    cf* __restrict__ x = BATCH ? p.x + bsrc * p.vox_stride : p.x;
     for (unsigned w = blockIdx.x * SLAB_THREADS + threadIdx.x; w < n_out; w += gridDim.x * SLAB_THREADS) {
         const unsigned item = w / TT;
         const int e = (int)(w - item * TT);
